@@ -1,0 +1,479 @@
+// ao_api.cu -- host side of libao.so: the extern "C" entry points declared in include/ao.h.
+// Validation, device tables, workspace planning and launch sequencing only; every number of
+// the forward model is produced by the kernels in k_*.cu.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "ao_internal.cuh"
+
+namespace ao {
+
+static thread_local std::string g_err = "";
+void set_error(const std::string& msg) { g_err = msg; }
+
+static int fail(int code, const std::string& msg) { set_error(msg); return code; }
+static int cuda_fail(cudaError_t e, const char* what)
+{
+    return fail(AO_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define AO_CUDA(call, what) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(e__, what); } while (0)
+
+static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+static int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+template <typename T>
+static cudaError_t upload(T** dptr, const T* host, size_t count)
+{
+    *dptr = nullptr;
+    if (count == 0) return cudaSuccess;
+    cudaError_t e = cudaMalloc((void**)dptr, sizeof(T) * count);
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dptr, host, sizeof(T) * count, cudaMemcpyHostToDevice);
+}
+
+static cudaError_t build_group(ao_geometry* g, Group& grp)
+{
+    std::vector<long long> off_api, off_stage;
+    long long acc = 0;
+    grp.max_N = 0;
+    for (int s : grp.src) {
+        const SourceP& sp = g->sources[s];
+        off_api.push_back(sp.phase_off);
+        off_stage.push_back(acc);
+        acc += (long long)sp.N * sp.N;
+        if (sp.N > grp.max_N) grp.max_N = sp.N;
+    }
+    grp.stage_elems = acc;
+    cudaError_t e;
+    if ((e = upload(&grp.d_src, grp.src.data(), grp.src.size())) != cudaSuccess) return e;
+    if ((e = upload(&grp.d_off_api, off_api.data(), off_api.size())) != cudaSuccess) return e;
+    return upload(&grp.d_off_stage, off_stage.data(), off_stage.size());
+}
+
+static void free_group(Group& grp)
+{
+    cudaFree(grp.d_src); cudaFree(grp.d_off_api); cudaFree(grp.d_off_stage);
+    grp.d_src = nullptr; grp.d_off_api = nullptr; grp.d_off_stage = nullptr;
+}
+
+static void destroy(ao_geometry* g)
+{
+    if (!g) return;
+    cudaFree(g->d_pupil_amp); cudaFree(g->d_layers); cudaFree(g->d_sources);
+    cudaFree(g->d_psf_tw); cudaFree(g->d_psf_pre);
+    for (auto& w : g->wfs) {
+        cudaFree(w.d_amp); cudaFree(w.d_valid); cudaFree(w.d_w2m); cudaFree(w.d_tw); cudaFree(w.d_pre);
+        free_group(w.grp);
+    }
+    free_group(g->all); free_group(g->sci);
+    delete g;
+}
+
+// ---- workspace planning ---------------------------------------------------------------------
+struct Plan {
+    size_t scratch = 0;     // FFT scratch (one step of the largest big transform batch)
+    size_t fixed = 0;       // PSF staging for ao_forward_host
+    size_t stage = 0;       // per step: phase staging (largest group)
+    size_t bigimg = 0;      // per step: images of the largest big WFS
+    size_t slopes = 0;      // per step: slopes of all WFS (ao_forward_host staging)
+    size_t per_step() const { return stage + bigimg + slopes; }
+};
+
+static Plan make_plan(const ao_geometry* g)
+{
+    Plan p;
+    size_t stage_elems = 0;
+    if (g->psf_fft && !g->sci.src.empty()) {
+        p.scratch = psf_scratch_bytes(g);
+        p.fixed = align256(sizeof(float) * g->sci.src.size() * (size_t)g->psf_fft * g->psf_fft);
+        stage_elems = (size_t)g->sci.stage_elems;
+    }
+    for (const auto& w : g->wfs) {
+        const size_t n_sel = w.grp.src.size(), nsa = (size_t)w.n_sub * w.n_sub;
+        if ((size_t)w.grp.stage_elems > stage_elems) stage_elems = (size_t)w.grp.stage_elems;
+        p.slopes += align256(sizeof(float) * n_sel * 2 * nsa);
+        if (w.big) {
+            const size_t s = sh_big_scratch_bytes(g, w);
+            if (s > p.scratch) p.scratch = s;
+            const size_t im = align256(sizeof(float) * n_sel * nsa * w.P * w.P);
+            if (im > p.bigimg) p.bigimg = im;
+        }
+    }
+    p.scratch = align256(p.scratch);
+    p.stage = align256(sizeof(float) * stage_elems);
+    return p;
+}
+
+struct WsView {
+    float2* scratch; float* psf_stage; float* stage; float* bigimg; float* slopes; int chunk;
+};
+
+static WsView ws_view(const ao_geometry* g)
+{
+    const Plan p = make_plan(g);
+    WsView v;
+    char* b = g->ws;
+    v.chunk = g->ws_chunk;
+    v.scratch = (float2*)b; b += p.scratch;
+    v.psf_stage = (float*)b; b += p.fixed;
+    v.stage = (float*)b; b += p.stage * (size_t)v.chunk;
+    v.bigimg = (float*)b; b += p.bigimg * (size_t)v.chunk;
+    v.slopes = (float*)b;
+    return v;
+}
+
+static NoiseP make_noise(const ao_noise* nz)
+{
+    NoiseP p; memset(&p, 0, sizeof(p));
+    if (nz) {
+        p.on = 1; p.key0 = (uint32_t)nz->seed; p.key1 = (uint32_t)(nz->seed >> 32);
+        p.photons = nz->photons_per_subap; p.read_noise = nz->read_noise_e;
+    }
+    return p;
+}
+
+static int check_entry(const ao_geometry* g)
+{
+    if (!g) return fail(AO_ERR_INVALID_ARG, "NULL handle");
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "pending CUDA error from earlier work");
+    return AO_OK;
+}
+
+// Run SH (+noise, +CoG) of WFS w for steps [step0, step0+n_steps), chunked by the workspace.
+static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0, int n_steps, double dt,
+                   const ao_noise* noise, float* images, float* slopes, cudaStream_t st)
+{
+    WfsH& w = g->wfs[wi];
+    const size_t n_sel = w.grp.src.size(), nsa = (size_t)w.n_sub * w.n_sub, PP = (size_t)w.P * w.P;
+    if (n_sel == 0) return AO_OK;
+    const bool need_ws = (phase_dev == nullptr) || w.big;
+    if (need_ws && (!g->ws || g->ws_chunk < 1))
+        return fail(AO_ERR_WORKSPACE, "workspace required (phase_dev == NULL or fft > 64): call ao_set_workspace");
+    const NoiseP nz = make_noise(noise);
+    const WsView v = need_ws ? ws_view(g) : WsView{};
+    const int chunk = need_ws ? v.chunk : n_steps;
+    for (int c0 = 0; c0 < n_steps; c0 += chunk) {
+        const int ks = (n_steps - c0 < chunk) ? n_steps - c0 : chunk;
+        const float* ph; bool api; long long stride;
+        if (phase_dev) {
+            ph = phase_dev + (size_t)c0 * g->phase_elems_per_step; api = true; stride = g->phase_elems_per_step;
+        } else {
+            AO_CUDA(launch_trace(g, w.grp, false, w.grp.stage_elems, step0 + c0, ks, dt, v.stage, st), "trace");
+            ph = v.stage; api = false; stride = w.grp.stage_elems;
+        }
+        float* img = images ? images + (size_t)c0 * n_sel * nsa * PP : nullptr;
+        float* slp = slopes ? slopes + (size_t)c0 * n_sel * 2 * nsa : nullptr;
+        if (!w.big) {
+            AO_CUDA(launch_sh_small(g, w, ph, api, stride, step0 + c0, ks, nz, img, slp, st), "sh_small");
+        } else {
+            float* im = img ? img : v.bigimg;
+            AO_CUDA(launch_sh_big(g, w, ph, api, stride, ks, v.scratch, im, st), "sh_big");
+            if (nz.on) AO_CUDA(launch_noise(g, w, im, step0 + c0, ks, nz, st), "noise");
+            if (slp) AO_CUDA(launch_centroids(g, w, im, ks * (int)n_sel, slp, st), "centroids");
+        }
+    }
+    return AO_OK;
+}
+
+static int run_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, double dt,
+                   float* psf, int accumulate, cudaStream_t st)
+{
+    if (g->sci.src.empty() || !g->psf_fft) return fail(AO_ERR_INVALID_ARG, "no science direction / psf_fft == 0");
+    if (!g->ws || g->ws_chunk < 1) return fail(AO_ERR_WORKSPACE, "ao_psf needs a workspace: call ao_set_workspace");
+    const WsView v = ws_view(g);
+    if (n_steps == 0 && !accumulate) {
+        AO_CUDA(cudaMemsetAsync(psf, 0, sizeof(float) * g->sci.src.size() * (size_t)g->psf_fft * g->psf_fft, st), "memset");
+        return AO_OK;
+    }
+    for (int c0 = 0; c0 < n_steps; c0 += v.chunk) {
+        const int ks = (n_steps - c0 < v.chunk) ? n_steps - c0 : v.chunk;
+        const float* ph; bool api; long long stride;
+        if (phase_dev) {
+            ph = phase_dev + (size_t)c0 * g->phase_elems_per_step; api = true; stride = g->phase_elems_per_step;
+        } else {
+            AO_CUDA(launch_trace(g, g->sci, false, g->sci.stage_elems, step0 + c0, ks, dt, v.stage, st), "trace");
+            ph = v.stage; api = false; stride = g->sci.stage_elems;
+        }
+        for (int k = 0; k < ks; ++k)
+            AO_CUDA(launch_psf(g, ph, api, stride, k, v.scratch, psf, (accumulate || c0 + k > 0) ? 1 : 0, st), "psf");
+    }
+    return AO_OK;
+}
+
+}  // namespace ao
+
+using namespace ao;
+
+extern "C" {
+
+const char* ao_last_error(void) { return g_err.c_str(); }
+const char* ao_version(void) { return "ao-forward-b200 0.1 (sm_100a)"; }
+
+int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, const ao_layer* layers,
+                       int n_layers, const ao_source* src, int n_src, double lambda_ref_m, int psf_fft,
+                       ao_geometry** out)
+{
+    if (out) *out = nullptr;
+    if (!out || !pupil || !pupil->amp_host || n_wfs < 0 || n_layers < 0 || n_src < 0 ||
+        (n_wfs > 0 && !wfs) || (n_layers > 0 && !layers) || (n_src > 0 && !src))
+        return fail(AO_ERR_INVALID_ARG, "ao_geometry_create: NULL pointer or negative count");
+    if (pupil->n <= 0 || !(pupil->pitch_m > 0) || !(lambda_ref_m > 0))
+        return fail(AO_ERR_SHAPE, "pupil n, pitch and lambda_ref must be positive");
+    if (n_layers > kMaxLayers) return fail(AO_ERR_UNSUPPORTED, "more than 128 layers");
+    for (int i = 0; i < n_wfs; ++i) {
+        const ao_wfs& w = wfs[i];
+        if (!w.amp_host) return fail(AO_ERR_INVALID_ARG, "wfs amp_host is NULL");
+        if (w.n_sub <= 0 || w.n_samp <= 0 || w.fft <= 0 || w.bin <= 0 || w.n_pix <= 0 || w.n_samp > w.fft ||
+            (w.fft & 1) || w.bin * w.n_pix > w.fft || ((w.fft - w.bin * w.n_pix) & 1))
+            return fail(AO_ERR_SHAPE, "wfs: need n_samp <= fft, fft even, bin*n_pix <= fft, (fft-bin*n_pix) even");
+        if (w.fft > 64) {
+            if (!is_pow2(w.fft) || w.fft > 4096) return fail(AO_ERR_UNSUPPORTED, "wfs fft > 64 must be a power of two <= 4096");
+            if ((size_t)w.bin * w.fft * sizeof(float2) > 200 * 1024)
+                return fail(AO_ERR_UNSUPPORTED, "wfs fft > 64: bin*fft*8 bytes must fit in 200 KB of shared memory");
+        }
+        if ((size_t)w.n_sub * w.n_sub > 65535u * 32u) return fail(AO_ERR_UNSUPPORTED, "too many subapertures");
+    }
+    for (int i = 0; i < n_layers; ++i) {
+        if (layers[i].n <= 1 || !(layers[i].pitch_m > 0)) return fail(AO_ERR_SHAPE, "layer n > 1 and pitch > 0 required");
+        if (!layers[i].screen_dev) return fail(AO_ERR_INVALID_ARG, "layer screen_dev is NULL");
+    }
+    for (int i = 0; i < n_src; ++i) {
+        if (src[i].wfs_index < -1 || src[i].wfs_index >= n_wfs) return fail(AO_ERR_INVALID_ARG, "source wfs_index out of range");
+        if (!(src[i].lambda_m > 0) || !(src[i].altitude_m > 0)) return fail(AO_ERR_SHAPE, "source lambda and altitude must be positive");
+    }
+    if (psf_fft != 0 && (!is_pow2(psf_fft) || psf_fft < 64 || psf_fft > 4096 || psf_fft < pupil->n))
+        return fail(AO_ERR_UNSUPPORTED, "psf_fft must be 0 or a power of two in [64, 4096] and >= pupil n");
+
+    int dev_count = 0;
+    AO_CUDA(cudaGetDeviceCount(&dev_count), "cudaGetDeviceCount");
+    if (dev_count <= 0) return fail(AO_ERR_CUDA, "no CUDA device");
+
+    ao_geometry* g = new ao_geometry();
+    cudaError_t e = cudaSuccess;
+    auto bail = [&](const char* what) { int rc = cuda_fail(e, what); destroy(g); return rc; };
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
+
+    g->Np = pupil->n; g->pitch = pupil->pitch_m; g->lambda_ref = lambda_ref_m;
+    const size_t np2 = (size_t)g->Np * g->Np;
+    for (size_t i = 0; i < np2; ++i) g->sumA2 += (double)pupil->amp_host[i] * pupil->amp_host[i];
+    if ((e = upload(&g->d_pupil_amp, pupil->amp_host, np2)) != cudaSuccess) return bail("pupil upload");
+
+    const double PI = 3.14159265358979323846;
+    g->layers.resize(n_layers);
+    for (int i = 0; i < n_layers; ++i) {
+        LayerP& lp = g->layers[i];
+        lp.screen = layers[i].screen_dev; lp.S = layers[i].n;
+        lp.mask = is_pow2(lp.S) ? lp.S - 1 : -1;
+        lp.inv_pitch = 1.0 / layers[i].pitch_m; lp.height = layers[i].height_m;
+        lp.wx = layers[i].wind_x_mps; lp.wy = layers[i].wind_y_mps;
+    }
+    if ((e = upload(&g->d_layers, g->layers.data(), g->layers.size())) != cudaSuccess) return bail("layers upload");
+
+    g->wfs.resize(n_wfs);
+    for (int i = 0; i < n_wfs; ++i) {
+        WfsH& w = g->wfs[i];
+        w.n_sub = wfs[i].n_sub; w.n = wfs[i].n_samp; w.M = wfs[i].fft; w.beta = wfs[i].bin; w.P = wfs[i].n_pix;
+        w.min_illum = wfs[i].min_illum; w.big = w.M > 64; w.logM = ilog2(w.M);
+        const int N = w.n_sub * w.n;
+        const float* A = wfs[i].amp_host;
+        w.valid.assign((size_t)w.n_sub * w.n_sub, 0);
+        for (int p = 0; p < w.n_sub; ++p)
+            for (int q = 0; q < w.n_sub; ++q) {
+                double s = 0;
+                for (int a = 0; a < w.n; ++a)
+                    for (int b = 0; b < w.n; ++b) { const double v = A[(size_t)(p * w.n + a) * N + q * w.n + b]; s += v * v; }
+                const bool ok = s / ((double)w.n * w.n) >= (double)w.min_illum;
+                w.valid[(size_t)p * w.n_sub + q] = ok; w.n_valid += ok;
+            }
+        if ((e = upload(&w.d_amp, A, (size_t)N * N)) != cudaSuccess) return bail("wfs amp upload");
+        if ((e = upload(&w.d_valid, w.valid.data(), w.valid.size())) != cudaSuccess) return bail("wfs valid upload");
+        if (!w.big) {
+            std::vector<float2> t(2 * w.M);
+            for (int q = 0; q < 2 * w.M; ++q) t[q] = make_float2((float)cos(PI * q / w.M), (float)(-sin(PI * q / w.M)));
+            if ((e = upload(&w.d_w2m, t.data(), t.size())) != cudaSuccess) return bail("twiddle upload");
+        } else {
+            std::vector<float2> t(w.M / 2), pr(w.n);
+            for (int k = 0; k < w.M / 2; ++k) t[k] = make_float2((float)cos(2 * PI * k / w.M), (float)(-sin(2 * PI * k / w.M)));
+            for (int a = 0; a < w.n; ++a) {
+                const long long q = ((long long)(w.M - 1) * a) % (2LL * w.M);     // exp(+i pi (M-1) a / M)
+                pr[a] = make_float2((float)cos(PI * (double)q / w.M), (float)sin(PI * (double)q / w.M));
+            }
+            if ((e = upload(&w.d_tw, t.data(), t.size())) != cudaSuccess) return bail("twiddle upload");
+            if ((e = upload(&w.d_pre, pr.data(), pr.size())) != cudaSuccess) return bail("pre-twiddle upload");
+        }
+    }
+
+    g->sources.resize(n_src);
+    long long off = 0;
+    const double width = (double)g->Np * g->pitch;
+    for (int i = 0; i < n_src; ++i) {
+        SourceP& sp = g->sources[i];
+        sp.wfs = src[i].wfs_index;
+        sp.N = sp.wfs < 0 ? g->Np : g->wfs[sp.wfs].n_sub * g->wfs[sp.wfs].n;
+        sp.d = width / (double)sp.N;
+        sp.thx = src[i].theta_x_rad; sp.thy = src[i].theta_y_rad;
+        sp.H = src[i].altitude_m; sp.inv_H = std::isinf(sp.H) ? 0.0 : 1.0 / sp.H;
+        sp.scale = lambda_ref_m / src[i].lambda_m;
+        sp.phase_off = off;
+        off += (long long)sp.N * sp.N;
+        g->all.src.push_back(i);
+        if (sp.wfs < 0) g->sci.src.push_back(i); else g->wfs[sp.wfs].grp.src.push_back(i);
+    }
+    g->phase_elems_per_step = off;
+    if ((e = upload(&g->d_sources, g->sources.data(), g->sources.size())) != cudaSuccess) return bail("sources upload");
+    if ((e = build_group(g, g->all)) != cudaSuccess) return bail("group upload");
+    if ((e = build_group(g, g->sci)) != cudaSuccess) return bail("group upload");
+    for (auto& w : g->wfs) if ((e = build_group(g, w.grp)) != cudaSuccess) return bail("group upload");
+
+    g->psf_fft = psf_fft;
+    if (psf_fft) {
+        g->psf_log = ilog2(psf_fft);
+        std::vector<float2> t(psf_fft / 2), pr(g->Np);
+        for (int k = 0; k < psf_fft / 2; ++k) t[k] = make_float2((float)cos(2 * PI * k / psf_fft), (float)(-sin(2 * PI * k / psf_fft)));
+        for (int a = 0; a < g->Np; ++a) pr[a] = make_float2((a & 1) ? -1.0f : 1.0f, 0.0f);
+        if ((e = upload(&g->d_psf_tw, t.data(), t.size())) != cudaSuccess) return bail("psf twiddle upload");
+        if ((e = upload(&g->d_psf_pre, pr.data(), pr.size())) != cudaSuccess) return bail("psf pre upload");
+    }
+    *out = g;
+    return AO_OK;
+}
+
+int ao_geometry_destroy(ao_geometry* g)
+{
+    if (!g) return AO_OK;
+    cudaDeviceSynchronize();
+    destroy(g);
+    return AO_OK;
+}
+
+size_t ao_workspace_bytes(const ao_geometry* g, int max_steps)
+{
+    if (!g) return 0;
+    if (max_steps < 1) max_steps = 1;
+    const Plan p = make_plan(g);
+    const size_t per = p.per_step();
+    size_t chunk = (size_t)max_steps;
+    const size_t cap = (size_t)1 << 30;                      // keep the per-chunk staging near 1 GiB
+    if (per > 0 && chunk * per > cap) chunk = cap / per > 0 ? cap / per : 1;
+    return p.scratch + p.fixed + chunk * per + 256;
+}
+
+int ao_set_workspace(ao_geometry* g, void* workspace_dev, size_t bytes)
+{
+    if (!g) return fail(AO_ERR_INVALID_ARG, "NULL handle");
+    g->ws = nullptr; g->ws_bytes = 0; g->ws_chunk = 0;
+    if (!workspace_dev) return AO_OK;
+    if (((uintptr_t)workspace_dev & 255) != 0) return fail(AO_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    const Plan p = make_plan(g);
+    const size_t base = p.scratch + p.fixed, per = p.per_step();
+    if (bytes < base + per) return fail(AO_ERR_WORKSPACE, "workspace smaller than ao_workspace_bytes(g, 1)");
+    g->ws = (char*)workspace_dev; g->ws_bytes = bytes;
+    const size_t c = per ? (bytes - base) / per : 1u << 20;
+    g->ws_chunk = (int)(c > (1u << 20) ? (1u << 20) : c);
+    return AO_OK;
+}
+
+size_t ao_phase_elems_per_step(const ao_geometry* g) { return g ? (size_t)g->phase_elems_per_step : 0; }
+
+size_t ao_phase_offset(const ao_geometry* g, int source, int step)
+{
+    if (!g || source < 0 || source >= (int)g->sources.size() || step < 0) return (size_t)-1;
+    return (size_t)step * (size_t)g->phase_elems_per_step + (size_t)g->sources[source].phase_off;
+}
+
+int ao_wfs_valid(const ao_geometry* g, int wfs_index, uint8_t* valid_host)
+{
+    if (!g || wfs_index < 0 || wfs_index >= (int)g->wfs.size()) return -1;
+    const WfsH& w = g->wfs[wfs_index];
+    if (valid_host) memcpy(valid_host, w.valid.data(), w.valid.size());
+    return w.n_valid;
+}
+
+int64_t ao_launch_count(const ao_geometry* g) { return g ? g->launches : 0; }
+
+int ao_trace_layers(ao_geometry* g, int64_t step0, int n_steps, double dt_s, float* phase_dev, void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (!phase_dev || n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_trace_layers: phase_dev NULL or n_steps < 0");
+    AO_CUDA(launch_trace(g, g->all, true, g->phase_elems_per_step, step0, n_steps, dt_s, phase_dev,
+                         (cudaStream_t)cuda_stream), "trace");
+    return AO_OK;
+}
+
+int ao_sh_images(ao_geometry* g, int wfs_index, const float* phase_dev, int64_t step0, int n_steps,
+                 double dt_s, const ao_noise* noise, float* images_dev, float* slopes_dev, void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (wfs_index < 0 || wfs_index >= (int)g->wfs.size()) return fail(AO_ERR_INVALID_ARG, "ao_sh_images: wfs_index out of range");
+    if (n_steps < 0 || (!images_dev && !slopes_dev)) return fail(AO_ERR_INVALID_ARG, "ao_sh_images: n_steps < 0 or no output buffer");
+    return run_wfs(g, wfs_index, phase_dev, step0, n_steps, dt_s, noise, images_dev, slopes_dev, (cudaStream_t)cuda_stream);
+}
+
+int ao_centroids(ao_geometry* g, int wfs_index, const float* images_dev, int n_image_sets, float* slopes_dev,
+                 void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (wfs_index < 0 || wfs_index >= (int)g->wfs.size()) return fail(AO_ERR_INVALID_ARG, "ao_centroids: wfs_index out of range");
+    if (!images_dev || !slopes_dev || n_image_sets < 0) return fail(AO_ERR_INVALID_ARG, "ao_centroids: NULL buffer or negative count");
+    AO_CUDA(launch_centroids(g, g->wfs[wfs_index], images_dev, n_image_sets, slopes_dev, (cudaStream_t)cuda_stream), "centroids");
+    return AO_OK;
+}
+
+int ao_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, double dt_s, float* psf_dev,
+           int accumulate, void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (!psf_dev || n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_psf: psf_dev NULL or n_steps < 0");
+    return run_psf(g, phase_dev, step0, n_steps, dt_s, psf_dev, accumulate, (cudaStream_t)cuda_stream);
+}
+
+int ao_forward_host(ao_geometry* g, const float* const* screens_host, int64_t step0, int n_steps, double dt_s,
+                    const ao_noise* noise, float* const* slopes_host, float* psf_host, void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_forward_host: n_steps < 0");
+    if (!g->ws || g->ws_chunk < 1) return fail(AO_ERR_WORKSPACE, "ao_forward_host needs a workspace");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (screens_host)
+        for (size_t l = 0; l < g->layers.size(); ++l) {
+            if (!screens_host[l]) return fail(AO_ERR_INVALID_ARG, "ao_forward_host: screens_host[l] is NULL");
+            AO_CUDA(cudaMemcpyAsync((void*)g->layers[l].screen, screens_host[l],
+                                    sizeof(float) * (size_t)g->layers[l].S * g->layers[l].S, cudaMemcpyHostToDevice, st), "screen upload");
+        }
+    const WsView v = ws_view(g);
+    if (slopes_host) {
+        for (int c0 = 0; c0 < n_steps; c0 += v.chunk) {
+            const int ks = (n_steps - c0 < v.chunk) ? n_steps - c0 : v.chunk;
+            char* sl = (char*)v.slopes;
+            for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
+                const WfsH& w = g->wfs[wi];
+                const size_t per = sizeof(float) * w.grp.src.size() * 2 * (size_t)w.n_sub * w.n_sub;
+                float* dst = (float*)sl;
+                sl += align256(per) * (size_t)v.chunk;
+                if (!slopes_host[wi] || w.grp.src.empty()) continue;
+                rc = run_wfs(g, (int)wi, nullptr, step0 + c0, ks, dt_s, noise, nullptr, dst, st);
+                if (rc) return rc;
+                AO_CUDA(cudaMemcpyAsync((char*)slopes_host[wi] + per * (size_t)c0, dst, per * (size_t)ks,
+                                        cudaMemcpyDeviceToHost, st), "slopes download");
+            }
+        }
+    }
+    if (psf_host && g->psf_fft && !g->sci.src.empty()) {
+        rc = run_psf(g, nullptr, step0, n_steps, dt_s, v.psf_stage, 0, st);
+        if (rc) return rc;
+        AO_CUDA(cudaMemcpyAsync(psf_host, v.psf_stage, sizeof(float) * g->sci.src.size() * (size_t)g->psf_fft * g->psf_fft,
+                                cudaMemcpyDeviceToHost, st), "psf download");
+    }
+    AO_CUDA(cudaStreamSynchronize(st), "stream synchronize");
+    return AO_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,58 @@
+// ao_device.cuh -- small device helpers shared by the CUDA kernels (noise model O5, reductions).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "ao_internal.cuh"
+
+namespace ao {
+
+// Philox4x32-10 (Salmon et al., SC'11), restated for the device: ten rounds of
+//   (c0,c1,c2,c3) <- (hi(M1 c2)^c1^k0, lo(M1 c2), hi(M0 c0)^c3^k1, lo(M0 c0)), key += (W0, W1).
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1)
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c.x), lo0 = M0 * c.x;
+        const uint32_t hi1 = __umulhi(M1, c.z), lo1 = M1 * c.z;
+        c = make_uint4(hi1 ^ c.y ^ k0, lo1, hi0 ^ c.w ^ k1, lo0);
+        k0 += W0; k1 += W1;
+    }
+    return c;
+}
+
+// u = ((w >> 8) + 0.5) 2^-24, exact in fp32.
+__device__ __forceinline__ float u24(uint32_t w) { return ((float)(w >> 8) + 0.5f) * (1.0f / 16777216.0f); }
+
+// Detector pixel with noise (reading O5): Poisson(mu) by sequential-search inversion of the
+// CDF plus read_noise * N(0,1) (Box-Muller).  The CDF search runs in FP64: exp(-mu) underflows
+// fp32 for mu > 87 and the integer decision must not depend on fp32 rounding of the CDF.
+__device__ __forceinline__ float noisy_pixel(float I, const NoiseP& nz, uint32_t px, uint32_t sa,
+                                             uint32_t src, uint32_t step)
+{
+    const uint4 w = philox4x32_10(make_uint4(px, sa, src, step), nz.key0, nz.key1);
+    const double mu = (double)(nz.photons * I);
+    int k = 0;
+    if (mu > 0.0) {
+        const double u = (double)u24(w.x);
+        double p = exp(-mu), c = p;
+        while (u > c && k < 100000) {
+            ++k;
+            p *= mu / (double)k;
+            c += p;
+            if (p == 0.0 && (double)k > mu) break;
+        }
+    }
+    const float z = sqrtf(-2.0f * logf(u24(w.y))) * cospif(2.0f * u24(w.z));
+    return fmaf(nz.read_noise, z, (float)k);
+}
+
+__device__ __forceinline__ float warp_sum(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+}  // namespace ao

@@ -1,0 +1,122 @@
+// ao_internal.cuh -- internal declarations of libao.so (CUDA path only; the oracle shares nothing with it).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "ao.h"
+
+namespace ao {
+
+constexpr int kMaxLayers = 128;
+
+// Per-layer parameters in device memory (one array per handle).
+struct LayerP {
+    const float* screen;   // [S][S]
+    int S;
+    int mask;              // S-1 if S is a power of two, else -1 (use %)
+    double inv_pitch;      // 1/d_l
+    double height;         // h_l
+    double wx, wy;         // wind m/s
+};
+
+// Per-source parameters in device memory.
+struct SourceP {
+    int N;                 // grid samples per side
+    int wfs;               // wfs index or -1
+    double d;              // grid pitch d_s
+    double thx, thy;       // direction (rad)
+    double H;              // altitude (inf for NGS/science)
+    double inv_H;          // 1/H (0 for inf)
+    double scale;          // lambda_ref / lambda_s
+    long long phase_off;   // element offset inside one step of the caller's phase buffer
+};
+
+// A group of sources processed together (all / those of one WFS / science directions).
+struct Group {
+    std::vector<int> src;          // global source indices, ascending
+    int* d_src = nullptr;          // device copy
+    long long* d_off_api = nullptr;   // phase offsets in the API layout (per member)
+    long long* d_off_stage = nullptr; // phase offsets in the compact staging layout (per member)
+    long long stage_elems = 0;     // elements per step in the staging layout
+    int max_N = 0;
+};
+
+struct NoiseP {
+    int on;
+    uint32_t key0, key1;
+    float photons, read_noise;
+};
+
+struct WfsH {
+    int n_sub, n, M, beta, P;
+    float min_illum;
+    bool big;                       // M > 64: multi-pass HBM FFT
+    int logM = 0;
+    float* d_amp = nullptr;         // [N][N]
+    uint8_t* d_valid = nullptr;     // [n_sub^2]
+    std::vector<uint8_t> valid;
+    int n_valid = 0;
+    float2* d_w2m = nullptr;        // W[q] = exp(-i pi q / M), q < 2M     (small path)
+    float2* d_tw = nullptr;         // exp(-2 pi i k / M), k < M/2         (big path)
+    float2* d_pre = nullptr;        // pre-twiddle exp(+i pi (M-1) a / M), a < n  (big path)
+    Group grp;
+};
+
+}  // namespace ao
+
+struct ao_geometry {
+    int Np = 0;
+    double pitch = 0;
+    float* d_pupil_amp = nullptr;
+    double sumA2 = 0;
+    std::vector<ao::WfsH> wfs;
+    std::vector<ao::LayerP> layers;
+    ao::LayerP* d_layers = nullptr;
+    std::vector<ao::SourceP> sources;
+    ao::SourceP* d_sources = nullptr;
+    double lambda_ref = 0;
+    int psf_fft = 0, psf_log = 0;
+    float2* d_psf_tw = nullptr;
+    float2* d_psf_pre = nullptr;      // (-1)^a as a complex table, a < Np
+    ao::Group all, sci;
+    long long phase_elems_per_step = 0;
+    // workspace
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    int ws_chunk = 0;                 // steps per internal chunk that fit the workspace
+    int64_t launches = 0;
+    int sm_count = 148;
+};
+
+namespace ao {
+
+// ---- kernel launchers (each returns the cudaError of the launch) ----
+cudaError_t launch_trace(ao_geometry* g, const Group& grp, bool api_layout, long long step_stride,
+                         int64_t step0, int n_steps, double dt, float* phase, cudaStream_t st);
+
+cudaError_t launch_sh_small(ao_geometry* g, const WfsH& w, const float* phase, bool api_layout,
+                            long long step_stride, int64_t step0, int n_steps, const NoiseP& noise,
+                            float* images, float* slopes, cudaStream_t st);
+
+cudaError_t launch_centroids(ao_geometry* g, const WfsH& w, const float* images, int n_sets,
+                             float* slopes, cudaStream_t st);
+
+cudaError_t launch_noise(ao_geometry* g, const WfsH& w, float* images, int64_t step0, int n_steps,
+                         const NoiseP& noise, cudaStream_t st);
+
+// big FFT: SH mode for one step-chunk of WFS w (images out), PSF mode for one step (psf +=).
+cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, bool api_layout,
+                          long long step_stride, int n_steps, float2* scratch, float* images,
+                          cudaStream_t st);
+cudaError_t launch_psf(ao_geometry* g, const float* phase, bool api_layout, long long step_stride,
+                       int step_in_chunk, float2* scratch, float* psf, int accumulate,
+                       cudaStream_t st);
+
+size_t sh_big_scratch_bytes(const ao_geometry* g, const WfsH& w);   // per step
+size_t psf_scratch_bytes(const ao_geometry* g);                      // per step
+
+void set_error(const std::string& msg);
+
+}  // namespace ao

@@ -1,0 +1,274 @@
+"""GPU-vs-oracle parity through the C ABI (pytest -m gpu; runs on the B200 box).
+
+Sizes are chosen so the FP64 oracle finishes in seconds while the inputs still span several
+CTAs/tiles and ragged tails (subaperture grids that are not multiples of the CTA batch,
+pupils not multiples of 32).  Tolerances: BASELINE.json north_star (tests/parity_util.py).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1608_00386_b200 import inputs
+from tests.parity_util import IMAGE_TOL, PHASE_TOL, SLOPE_TOL, check_wfs, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+def _geo(cfg, steps=1):
+    from paper_1608_00386_b200 import binding
+    return binding.Geometry(cfg, workspace_steps=steps)
+
+
+def _run_all(cfg, n_steps, step0=0):
+    """Unfused API path: trace -> phase -> sh_images / psf.  Returns torch outputs."""
+    import torch
+    geo = _geo(cfg, n_steps)
+    phase = geo.trace_layers(step0, n_steps, cfg.dt_s)
+    out = {"phase": phase, "geo": geo, "images": {}, "slopes": {}}
+    for w in range(len(cfg.wfs)):
+        if cfg.sources_of_wfs(w):
+            out["images"][w], out["slopes"][w] = geo.sh_images(w, phase, step0, n_steps, cfg.dt_s)
+    if cfg.psf_fft and cfg.science_sources():
+        out["psf"] = geo.psf(phase, step0, n_steps, cfg.dt_s)
+    torch.cuda.synchronize()
+    return out
+
+
+def _check_phase(cfg, geo, phase, ref, n_steps):
+    worst = 0.0
+    for s in range(len(cfg.sources)):
+        for k in range(n_steps):
+            got = geo.phase_view(phase, s, k).cpu().numpy()
+            worst = max(worst, rel_l2(got, ref["phase"][s][k]))
+    assert worst <= PHASE_TOL, f"phase rel L2 {worst:.3e}"
+    return worst
+
+
+def _check_all(cfg, n_steps, step0=0):
+    ref = oracle.forward(cfg, step0, n_steps)
+    out = _run_all(cfg, n_steps, step0)
+    geo = out["geo"]
+    _check_phase(cfg, geo, out["phase"], ref, n_steps)
+    for w in out["images"]:
+        assert np.array_equal(geo.wfs_valid(w), ref["valid"][w])
+        check_wfs(cfg, geo, ref, w, out["images"][w], out["slopes"][w], n_steps, cfg.name)
+    if "psf" in out:
+        for di, s in enumerate(cfg.science_sources()):
+            e = rel_l2(out["psf"][di].cpu().numpy(), ref["psf"][s])
+            assert e <= IMAGE_TOL, f"psf rel L2 {e:.3e}"
+    # fused path (phase_dev = NULL): same outputs without a phase buffer
+    for w in out["images"]:
+        img, slp = geo.sh_images(w, None, step0, n_steps, cfg.dt_s)
+        check_wfs(cfg, geo, ref, w, img, slp, n_steps, cfg.name + " fused")
+        _, slp2 = geo.sh_images(w, None, step0, n_steps, cfg.dt_s, want_images=False)
+        check_wfs(cfg, geo, ref, w, None, slp2, n_steps, cfg.name + " fused slopes-only")
+    if "psf" in out:
+        p2 = geo.psf(None, step0, n_steps, cfg.dt_s)
+        for di, s in enumerate(cfg.science_sources()):
+            assert rel_l2(p2[di].cpu().numpy(), ref["psf"][s]) <= IMAGE_TOL
+    return out, ref
+
+
+def test_c0_tiny_ngs_scao_full():
+    cfg = inputs.make_config(0)
+    _check_all(cfg, 1)
+
+
+def test_c1_elt_ngs_scao_reduced_three_steps():
+    # M = 24 (not a power of two), annular pupil, 3 layers, sub-pixel wind shift of 0.5 px/step
+    cfg = inputs.make_config(1, n_sub=18, screen_n=512, n_steps=3)
+    _check_all(cfg, 3, step0=5)
+
+
+def test_c2_maory_lgs_reduced_noiseless():
+    # 6 LGS with cone effect, 10 layers, off-axis, n_sub = 14 (ragged against any CTA batch)
+    cfg = inputs.make_config(2, n_sub=14, screen_n=512, n_steps=2)
+    _check_all(cfg, 2, step0=49)
+
+
+def test_c3_full_mcao_reduced_long_exposure():
+    # LGS + NGS (big FFT path, M = 128) + 10 science PSFs (M = 256) accumulated over 3 steps
+    cfg = inputs.make_config(3, n_sub=8, screen_n=512, n_steps=3)
+    assert cfg.wfs[1].fft == 128 and cfg.psf_fft == 256
+    _check_all(cfg, 3)
+
+
+@pytest.mark.parametrize("M", [16, 32, 64])
+def test_c4_throughput_sweep_reduced(M):
+    cfg = inputs.make_config(4, n_sub=10, screen_n=1024, n_steps=2, lgs_fft=M)
+    assert len(cfg.layers) == 35
+    _check_all(cfg, 2, step0=499)
+
+
+def test_c2_noise_protocol():
+    """Reading O5: identical Poisson counts on >= 1-1e-5 of the pixels; slopes within 1e-4 on
+    subapertures whose counts all agree; residual statistics match Poisson + read noise."""
+    import torch
+    cfg = inputs.make_config(2, n_sub=14, screen_n=512, n_steps=2)
+    n_steps = 2
+    ref = oracle.forward(cfg, 0, n_steps, want_psf=False, noise_on=True)
+    geo = _geo(cfg, n_steps)
+    phase = geo.trace_layers(0, n_steps, cfg.dt_s)
+    clean, _ = geo.sh_images(0, phase, 0, n_steps, cfg.dt_s)
+    noisy, slopes = geo.sh_images(0, phase, 0, n_steps, cfg.dt_s, noise=cfg.noise)
+    torch.cuda.synchronize()
+    ron = cfg.noise.read_noise_e
+    tot = bad = 0
+    worst = 0.0
+    resid, var = [], []
+    for si, s in enumerate(cfg.sources_of_wfs(0)):
+        for k in range(n_steps):
+            g = noisy[k, si].cpu().numpy().astype(np.float64)
+            r = ref["noisy"][s][k]
+            # the Gaussian part is continuous: |g - r| < 0.5 <=> same Poisson count
+            same = np.abs(g - r) < 0.5
+            tot += same.size; bad += int((~same).sum())
+            ok_sub = same.reshape(same.shape[0], -1).all(axis=1)
+            assert np.abs(g - r)[same].max() < 2e-3            # fp32 Box-Muller vs fp64
+            d = np.abs(slopes[k, si].cpu().numpy().astype(np.float64) - ref["slopes"][s][k])
+            worst = max(worst, d[:, ok_sub].max())
+            mu = cfg.noise.photons_per_subap * ref["images"][s][k]
+            v = ref["valid"][0].astype(bool)
+            resid.append((g - mu)[v].ravel()); var.append((mu + ron ** 2)[v].ravel())
+    assert bad <= max(1, int(1e-5 * tot)), f"{bad} of {tot} Poisson counts differ"
+    assert worst <= SLOPE_TOL
+    resid = np.concatenate(resid); var = np.concatenate(var)
+    assert abs(resid.sum() / math.sqrt(var.sum())) < 4.0
+    assert abs((resid ** 2 / var).mean() - 1.0) < 4.0 * math.sqrt(2.5 / resid.size)
+    # stand-alone noise path == fused path is not required; noiseless images unchanged
+    check_wfs(cfg, geo, ref, 0, clean, None, n_steps, "c2 clean")
+
+
+def test_noise_device_philox_matches_oracle_bits():
+    """Bright flat images, no read noise: GPU Poisson counts must equal the oracle's exactly
+    (same Philox words, same FP64 inverse-CDF search)."""
+    import torch
+    cfg = inputs.make_config(0, with_screens=False)
+    cfg.layers[0].screen = np.zeros((256, 256), np.float32)
+    nz = inputs.Noise(seed=0xDEADBEEF12345678, photons_per_subap=5000.0, read_noise_e=0.0)
+    geo = _geo(cfg, 1)
+    noisy, _ = geo.sh_images(0, None, 7, 1, cfg.dt_s, noise=nz)
+    torch.cuda.synchronize()
+    img, valid = oracle.sh_images(np.zeros((80, 80)), cfg.wfs[0].amp, 10, 8, 16, 2, 8, 0.5)
+    _, counts = oracle.noise(img, valid, nz.seed, 0, 7, nz.photons_per_subap, 0.0)
+    got = noisy[0, 0].cpu().numpy()
+    assert np.array_equal(got[valid.astype(bool)], counts[valid.astype(bool)].astype(np.float32))
+    assert counts.max() > 900      # mu ~ 1026 in the centre pixels: exp(-mu) underflows fp32
+
+
+def test_centroids_standalone_matches_oracle():
+    import torch
+    cfg = inputs.make_config(0, with_screens=False)
+    cfg.layers[0].screen = np.zeros((256, 256), np.float32)
+    geo = _geo(cfg, 1)
+    rng = np.random.default_rng(5)
+    imgs = rng.uniform(0.0, 1.0, (3, 100, 8, 8)).astype(np.float32)
+    imgs[1, 4] = 0.0                                    # zero-sum image -> slopes 0
+    s = geo.centroids(0, torch.from_numpy(imgs).cuda())
+    torch.cuda.synchronize()
+    valid = geo.wfs_valid(0)
+    for k in range(3):
+        ref = oracle.centroids(imgs[k].astype(np.float64), valid)
+        assert np.abs(s[k].cpu().numpy() - ref).max() <= 2e-6
+    assert float(s[1, 0, 4]) == 0.0 and float(s[1, 1, 4]) == 0.0
+
+
+def test_flat_wavefront_gives_zero_slopes_and_closed_form_image():
+    import torch
+    cfg = inputs.make_config(2, n_sub=6, screen_n=256, n_steps=1, with_screens=False)
+    for l in cfg.layers:
+        l.screen = np.full((256, 256), 3.25, np.float32)        # piston only
+    geo = _geo(cfg, 1)
+    img, slp = geo.sh_images(0, None, 0, 1, cfg.dt_s)
+    torch.cuda.synchronize()
+    valid = geo.wfs_valid(0).astype(bool)
+    assert float(slp.abs().max()) <= 2e-6
+    full = cfg.wfs[0].amp.reshape(6, 16, 6, 16).transpose(0, 2, 1, 3).reshape(36, 256).sum(1) == 256
+    prof = np.array([0.004116392250, 0.005814901476, 0.013954378208, 0.476114328066])
+    prof = np.concatenate([prof, prof[::-1]])                   # SURVEY.md section 8(c) c2 profile
+    got = img[0, 0].cpu().numpy()[full]
+    assert got.shape[0] > 0 and np.abs(got - np.outer(prof, prof)).max() < 2e-6
+    assert np.all(img[0, :, ~valid].cpu().numpy() == 0.0)
+
+
+def test_integer_pixel_shift_is_bit_exact_copy_and_periodic_wrap():
+    import torch
+    rng = np.random.default_rng(11)
+    S, N = 64, 16
+    scr = rng.standard_normal((S, S)).astype(np.float32)
+    pupil = inputs.Pupil(N, 0.5, 4.0, 0.0)
+    # wind 6 m/s along +x, -4 m/s along y, dt 0.25 s, pitch 0.5 m: 3 px and -2 px per step
+    cfg = inputs.Config("shift", pupil, [], [inputs.Layer(S, 0.5, 0.0, 6.0, -4.0, 1.0, scr)],
+                        [inputs.Source(0.0, 0.0, math.inf, 500e-9, -1)], 1, dt_s=0.25)
+    inputs.fill_masks(cfg)
+    geo = _geo(cfg, 1)
+    ph = geo.trace_layers(1, 1, cfg.dt_s)
+    torch.cuda.synchronize()
+    got = geo.phase_view(ph, 0, 0).cpu().numpy()
+    assert np.array_equal(got, scr[26:42, 21:37])
+    # 40 steps: footprint has wrapped around the 64-px screen more than once; still equals the oracle
+    ph = geo.trace_layers(40, 1, cfg.dt_s)
+    ref = oracle.trace(cfg.layers, 0, 0, math.inf, 500e-9, 500e-9, N, 0.5, 40 * 0.25)
+    assert np.array_equal(geo.phase_view(ph, 0, 0).cpu().numpy().astype(np.float64), ref)
+    # non power-of-two screen with a footprint larger than the screen (wraps inside one call)
+    scr2 = rng.standard_normal((48, 48)).astype(np.float32)
+    cfg2 = inputs.Config("wrap", inputs.Pupil(100, 0.1, 5.0, 0.0), [],
+                         [inputs.Layer(48, 0.13, 2000.0, 3.0, 1.0, 1.0, scr2)],
+                         [inputs.Source(1e-4, -2e-4, 90e3, 589e-9, -1)], 1)
+    inputs.fill_masks(cfg2)
+    geo2 = _geo(cfg2, 1)
+    ph2 = geo2.trace_layers(3, 2, cfg2.dt_s)
+    torch.cuda.synchronize()
+    for k in range(2):
+        ref = oracle.trace(cfg2.layers, 1e-4, -2e-4, 90e3, 589e-9, 500e-9, 100, 0.1, (3 + k) * cfg2.dt_s)
+        assert rel_l2(geo2.phase_view(ph2, 0, k).cpu().numpy(), ref) <= PHASE_TOL
+
+
+def test_empty_and_error_cases():
+    import torch
+    from paper_1608_00386_b200 import binding
+    cfg = inputs.make_config(0)
+    geo = _geo(cfg, 1)
+    # n_steps = 0 is a no-op
+    geo.trace_layers(0, 0, cfg.dt_s, phase=torch.empty(1, device="cuda"))
+    img, slp = geo.sh_images(0, None, 0, 0, cfg.dt_s)
+    assert img.numel() == 0
+    with pytest.raises(binding.AoError) as e:
+        geo.sh_images(3, None, 0, 1, cfg.dt_s)
+    assert e.value.status == 1
+    with pytest.raises(binding.AoError) as e:
+        geo.sh_images(0, None, 0, 1, cfg.dt_s, want_images=False, want_slopes=False)
+    assert e.value.status == 1
+    with pytest.raises(binding.AoError) as e:
+        geo.psf(None, 0, 1, cfg.dt_s, psf=torch.empty(4, device="cuda"))   # no science direction
+    assert e.value.status == 1
+    # layer above the source altitude is skipped; no layers at all gives flat phase
+    cfg2 = inputs.make_config(0, with_screens=False)
+    cfg2.layers = []
+    geo2 = _geo(cfg2, 1)
+    ph = geo2.trace_layers(0, 1, cfg2.dt_s)
+    torch.cuda.synchronize()
+    assert float(ph.abs().max()) == 0.0
+    assert geo.launch_count() > 0
+
+
+def test_forward_host_matches_device_path():
+    import torch
+    cfg = inputs.make_config(3, n_sub=8, screen_n=512, n_steps=3)
+    geo = _geo(cfg, 2)                                    # chunk of 2 steps < 3 steps: exercises chunking
+    ref = oracle.forward(cfg, 0, 3, want_phase=False)
+    sl = [torch.empty((3, len(cfg.sources_of_wfs(w)), 2, W.n_sub ** 2), dtype=torch.float32).pin_memory()
+          for w, W in enumerate(cfg.wfs)]
+    psf = torch.empty((len(cfg.science_sources()), cfg.psf_fft, cfg.psf_fft), dtype=torch.float32).pin_memory()
+    scr = [torch.from_numpy(l.screen).pin_memory() for l in cfg.layers]
+    for s in geo.screens:
+        s.zero_()                                          # the call must upload the screens itself
+    geo.forward_host(0, 3, cfg.dt_s, sl, psf, screens_host=scr)
+    for w in range(len(cfg.wfs)):
+        for si, s in enumerate(cfg.sources_of_wfs(w)):
+            for k in range(3):
+                assert np.abs(sl[w][k, si].numpy() - ref["slopes"][s][k]).max() <= SLOPE_TOL
+    for di, s in enumerate(cfg.science_sources()):
+        assert rel_l2(psf[di].numpy(), ref["psf"][s]) <= IMAGE_TOL
