@@ -126,7 +126,8 @@ class Geometry:
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         if screens is None:
-            screens = [torch.from_numpy(np.ascontiguousarray(l.screen, dtype=np.float32)).to(self.device)
+            screens = [l.screen_dev if getattr(l, "screen_dev", None) is not None else
+                       torch.from_numpy(np.ascontiguousarray(l.screen, dtype=np.float32)).to(self.device)
                        for l in cfg.layers]
         self.screens = screens
         fp = C.POINTER(C.c_float)
@@ -207,6 +208,8 @@ class Geometry:
     def sh_images(self, w: int, phase, step0: int, n_steps: int, dt_s: float, noise=None,
                   want_images=True, want_slopes=True, images=None, slopes=None):
         import torch
+        if not 0 <= w < len(self.cfg.wfs):       # let the library report the bad index
+            _check(self.lib.ao_sh_images(self.handle, w, None, step0, n_steps, dt_s, None, None, None, _stream()))
         W = self.cfg.wfs[w]
         n_sel = len(self.cfg.sources_of_wfs(w))
         nsa = W.n_sub * W.n_sub

@@ -402,7 +402,9 @@ int64_t ao_launch_count(const ao_geometry* g) { return g ? g->launches : 0; }
 int ao_trace_layers(ao_geometry* g, int64_t step0, int n_steps, double dt_s, float* phase_dev, void* cuda_stream)
 {
     int rc = check_entry(g); if (rc) return rc;
-    if (!phase_dev || n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_trace_layers: phase_dev NULL or n_steps < 0");
+    if (n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_trace_layers: n_steps < 0");
+    if (n_steps == 0) return AO_OK;
+    if (!phase_dev) return fail(AO_ERR_INVALID_ARG, "ao_trace_layers: phase_dev is NULL");
     AO_CUDA(launch_trace(g, g->all, true, g->phase_elems_per_step, step0, n_steps, dt_s, phase_dev,
                          (cudaStream_t)cuda_stream), "trace");
     return AO_OK;
@@ -413,7 +415,9 @@ int ao_sh_images(ao_geometry* g, int wfs_index, const float* phase_dev, int64_t 
 {
     int rc = check_entry(g); if (rc) return rc;
     if (wfs_index < 0 || wfs_index >= (int)g->wfs.size()) return fail(AO_ERR_INVALID_ARG, "ao_sh_images: wfs_index out of range");
-    if (n_steps < 0 || (!images_dev && !slopes_dev)) return fail(AO_ERR_INVALID_ARG, "ao_sh_images: n_steps < 0 or no output buffer");
+    if (n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_sh_images: n_steps < 0");
+    if (n_steps == 0) return AO_OK;
+    if (!images_dev && !slopes_dev) return fail(AO_ERR_INVALID_ARG, "ao_sh_images: no output buffer");
     return run_wfs(g, wfs_index, phase_dev, step0, n_steps, dt_s, noise, images_dev, slopes_dev, (cudaStream_t)cuda_stream);
 }
 

@@ -58,7 +58,8 @@ class Layer:
     wind_x_mps: float
     wind_y_mps: float
     weight: float            # Cn2 fraction (used by the generator only)
-    screen: Optional[np.ndarray] = None   # [n][n] float32 radians at LAMBDA_REF
+    screen: Optional[np.ndarray] = None   # [n][n] float32 radians at LAMBDA_REF (host copy)
+    screen_dev: Optional[object] = None   # the same screen as a torch CUDA tensor (keep_on_device)
 
 
 @dataclass
@@ -147,7 +148,7 @@ def screen_expected_variance(n: int, pitch_m: float, r0_m: float, L0_m: float) -
 
 
 def von_karman_pair(n: int, pitch_m: float, r0_m: float, L0_m: float,
-                    rng: np.random.Generator, device: str = "cpu"):
+                    rng: np.random.Generator, device: str = "cpu", as_torch: bool = False):
     """Two independent periodic von Karman screens [n][n] float32 (radians at 500 nm).
 
     c(f) = (xi1 + i xi2) sqrt(Phi(f)) df, c(0) = 0, phi = n^2 ifft2(c); Re and Im are
@@ -176,25 +177,45 @@ def von_karman_pair(n: int, pitch_m: float, r0_m: float, L0_m: float,
     del xi, amp, f2
     phi = torch.fft.ifft2(c) * float(n * n)
     del c
-    re = phi.real.to(torch.float32).cpu().numpy()
-    im = phi.imag.to(torch.float32).cpu().numpy()
-    return re, im
+    re = phi.real.to(torch.float32).contiguous()
+    im = phi.imag.to(torch.float32).contiguous()
+    del phi
+    if as_torch:
+        return re, im
+    return re.cpu().numpy(), im.cpu().numpy()
 
 
-def fill_screens(cfg: Config, device: str = "cpu") -> Config:
-    """Generate one screen per layer with r0_l = r0 w_l^(-3/5): each layer carries sqrt(weight)."""
+def fill_screens(cfg: Config, device: str = "cpu", keep_on_device: bool = False) -> Config:
+    """Generate one screen per layer with r0_l = r0 w_l^(-3/5): each layer carries sqrt(weight).
+
+    keep_on_device (device must be CUDA): leave the screens as torch CUDA tensors in
+    `screen_dev` (no host round trip for the 9.4 GB of c4); `screens_to_host` fetches them.
+    """
     rng = np.random.default_rng(np.random.PCG64(cfg.seed + 7919))
     spare = None
     for lay in cfg.layers:
         # r0_l^(-5/3) = r0^(-5/3) w_l, so a unit-weight screen times sqrt(w_l) is layer l's screen;
         # one FFT yields a pair (Re, Im): the spare serves the next layer of the same shape
         if spare is not None and spare[0] == (lay.n, lay.pitch_m):
-            lay.screen = (spare[1] * np.float32(math.sqrt(lay.weight))).astype(np.float32)
+            unit = spare[1]
             spare = None
         else:
-            a, b = von_karman_pair(lay.n, lay.pitch_m, cfg.r0_m, cfg.L0_m, rng, device)
-            lay.screen = (a * np.float32(math.sqrt(lay.weight))).astype(np.float32)
+            unit, b = von_karman_pair(lay.n, lay.pitch_m, cfg.r0_m, cfg.L0_m, rng, device,
+                                      as_torch=keep_on_device)
             spare = ((lay.n, lay.pitch_m), b)
+        if keep_on_device:
+            lay.screen_dev = unit * float(np.float32(math.sqrt(lay.weight)))   # fp32 tensor * python float
+            lay.screen = None
+        else:
+            lay.screen = (unit * np.float32(math.sqrt(lay.weight))).astype(np.float32)
+    return cfg
+
+
+def screens_to_host(cfg: Config) -> Config:
+    """Fill `screen` (numpy, host) from `screen_dev` for layers generated with keep_on_device."""
+    for lay in cfg.layers:
+        if lay.screen is None and lay.screen_dev is not None:
+            lay.screen = lay.screen_dev.cpu().numpy()
     return cfg
 
 
@@ -220,7 +241,7 @@ def _winds(rng: np.random.Generator, n_layers: int):
 def make_config(index: int, *, n_sub: Optional[int] = None, screen_n: Optional[int] = None,
                 n_steps: Optional[int] = None, lgs_fft: int = 32, ngs_samp: Optional[int] = None,
                 psf_fft: Optional[int] = None, n_layers: Optional[int] = None,
-                with_screens: bool = True, device: str = "cpu") -> Config:
+                with_screens: bool = True, device: str = "cpu", keep_on_device: bool = False) -> Config:
     """Build workload c<index> of BASELINE.json.
 
     The keyword overrides shrink a workload while keeping its recipe (same pitch, same
@@ -296,7 +317,7 @@ def make_config(index: int, *, n_sub: Optional[int] = None, screen_n: Optional[i
         raise ValueError("config index must be 0..4")
     fill_masks(cfg)
     if with_screens:
-        fill_screens(cfg, device=device)
+        fill_screens(cfg, device=device, keep_on_device=keep_on_device)
     return cfg
 
 
