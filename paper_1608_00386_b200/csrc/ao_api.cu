@@ -67,7 +67,7 @@ static void destroy(ao_geometry* g)
     cudaFree(g->d_pupil_amp); cudaFree(g->d_layers); cudaFree(g->d_sources);
     cudaFree(g->d_psf_tw); cudaFree(g->d_psf_pre);
     for (auto& w : g->wfs) {
-        cudaFree(w.d_amp); cudaFree(w.d_valid); cudaFree(w.d_w2m); cudaFree(w.d_tw); cudaFree(w.d_pre);
+        cudaFree(w.d_amp); cudaFree(w.d_valid); cudaFree(w.d_w2m); cudaFree(w.d_tw); cudaFree(w.d_pre); cudaFree(w.fused_items);
         free_group(w.grp);
     }
     free_group(g->all); free_group(g->sci);
@@ -152,6 +152,12 @@ static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0
     WfsH& w = g->wfs[wi];
     const size_t n_sel = w.grp.src.size(), nsa = (size_t)w.n_sub * w.n_sub, PP = (size_t)w.P * w.P;
     if (n_sel == 0) return AO_OK;
+    if (!phase_dev && !w.big) {                       // hot path: one fused kernel, no phase in HBM, no workspace
+        if (fused_supported(g, w)) {
+            AO_CUDA(launch_fused(g, w, step0, n_steps, dt, make_noise(noise), images, slopes, st), "fused");
+            return AO_OK;
+        }
+    }
     const bool need_ws = (phase_dev == nullptr) || w.big;
     if (need_ws && (!g->ws || g->ws_chunk < 1))
         return fail(AO_ERR_WORKSPACE, "workspace required (phase_dev == NULL or fft > 64): call ao_set_workspace");
@@ -295,6 +301,31 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
             }
         if ((e = upload(&w.d_amp, A, (size_t)N * N)) != cudaSuccess) return bail("wfs amp upload");
         if ((e = upload(&w.d_valid, w.valid.data(), w.valid.size())) != cudaSuccess) return bail("wfs valid upload");
+        fused_tile_shape(w.M, &w.fused_G, &w.fused_R2);
+        if (w.fused_G > 0) {
+            // work items of the fused kernel: for each band of fused_R2 subaperture rows, runs of at most
+            // fused_G adjacent columns in which at least one subaperture of the band is valid
+            std::vector<int> items;
+            for (int p = 0; p < w.n_sub; p += w.fused_R2) {
+                auto need = [&](int q) {
+                    for (int h = 0; h < w.fused_R2 && p + h < w.n_sub; ++h)
+                        if (w.valid[(size_t)(p + h) * w.n_sub + q]) return true;
+                    return false;
+                };
+                int q = 0;
+                while (q < w.n_sub) {
+                    if (!need(q)) { ++q; continue; }
+                    int cnt = 0;
+                    while (q + cnt < w.n_sub && cnt < w.fused_G && need(q + cnt)) ++cnt;
+                    items.push_back(p); items.push_back(q); items.push_back(cnt); items.push_back(0);
+                    q += cnt;
+                }
+            }
+            w.n_fused_items = (int)(items.size() / 4);
+            int* d = nullptr;
+            if ((e = upload(&d, items.data(), items.size())) != cudaSuccess) return bail("fused items upload");
+            w.fused_items = d;
+        }
         if (!w.big) {
             std::vector<float2> t(2 * w.M);
             for (int q = 0; q < 2 * w.M; ++q) t[q] = make_float2((float)cos(PI * q / w.M), (float)(-sin(PI * q / w.M)));

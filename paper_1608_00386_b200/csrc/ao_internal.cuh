@@ -61,6 +61,8 @@ struct WfsH {
     float2* d_w2m = nullptr;        // W[q] = exp(-i pi q / M), q < 2M     (small path)
     float2* d_tw = nullptr;         // exp(-2 pi i k / M), k < M/2         (big path)
     float2* d_pre = nullptr;        // pre-twiddle exp(+i pi (M-1) a / M), a < n  (big path)
+    void* fused_items = nullptr;    // device WorkItem[]: runs of <= fused_G adjacent valid subapertures
+    int n_fused_items = 0, fused_G = 0, fused_R2 = 0;
     Group grp;
 };
 
@@ -113,6 +115,12 @@ cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, boo
 cudaError_t launch_psf(ao_geometry* g, const float* phase, bool api_layout, long long step_stride,
                        int step_in_chunk, float2* scratch, float* psf, int accumulate,
                        cudaStream_t st);
+
+// fused trace + SH + CoG (k_fused.cu); cudaErrorNotSupported if the geometry is outside its fast path
+bool fused_supported(const ao_geometry* g, const WfsH& w);
+cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_steps, double dt,
+                         const NoiseP& noise, float* images, float* slopes, cudaStream_t st);
+void fused_tile_shape(int M, int* G, int* R2);
 
 size_t sh_big_scratch_bytes(const ao_geometry* g, const WfsH& w);   // per step
 size_t psf_scratch_bytes(const ao_geometry* g);                      // per step
