@@ -121,6 +121,9 @@ bool fused_supported(const ao_geometry* g, const WfsH& w);
 cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_steps, double dt,
                          const NoiseP& noise, float* images, float* slopes, cudaStream_t st);
 void fused_tile_shape(int M, int* G, int* R2);
+// tiled ray-trace into a phase buffer (k_fused.cu); cudaErrorNotSupported if outside its fast path
+cudaError_t launch_trace_tiled(ao_geometry* g, const Group& grp, bool api_layout, long long step_stride,
+                               int64_t step0, int n_steps, double dt, float* phase, cudaStream_t st);
 
 size_t sh_big_scratch_bytes(const ao_geometry* g, const WfsH& w);   // per step
 size_t psf_scratch_bytes(const ao_geometry* g);                      // per step

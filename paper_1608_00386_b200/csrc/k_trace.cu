@@ -75,6 +75,10 @@ cudaError_t launch_trace(ao_geometry* g, const Group& grp, bool api_layout, long
 {
     const int n_sel = (int)grp.src.size();
     if (n_sel == 0 || n_steps <= 0) return cudaSuccess;
+    {   // fast path: TMA-staged tiles (k_fused.cu); falls through for geometries it does not cover
+        const cudaError_t e = launch_trace_tiled(g, grp, api_layout, step_stride, step0, n_steps, dt, phase, st);
+        if (e != cudaErrorNotSupported) return e;
+    }
     dim3 block(32, 8, 1);
     const int gx = (grp.max_N + 31) / 32, gy = (grp.max_N + 7) / 8;
     // blockIdx.z is limited to 65535: split the step range if needed
