@@ -67,7 +67,7 @@ static void destroy(ao_geometry* g)
     cudaFree(g->d_pupil_amp); cudaFree(g->d_layers); cudaFree(g->d_sources);
     cudaFree(g->d_psf_tw); cudaFree(g->d_psf_pre);
     for (auto& w : g->wfs) {
-        cudaFree(w.d_amp); cudaFree(w.d_valid); cudaFree(w.d_w2m); cudaFree(w.d_tw); cudaFree(w.d_pre); cudaFree(w.fused_items);
+        cudaFree(w.d_amp); cudaFree(w.d_valid); cudaFree(w.d_w2m); cudaFree(w.d_tw); cudaFree(w.d_twf); cudaFree(w.d_pre); cudaFree(w.fused_items);
         free_group(w.grp);
     }
     free_group(g->all); free_group(g->sci);
@@ -89,7 +89,7 @@ static Plan make_plan(const ao_geometry* g)
     Plan p;
     size_t stage_elems = 0;
     if (g->psf_fft && !g->sci.src.empty()) {
-        p.scratch = psf_scratch_bytes(g);
+        p.scratch = psf_scratch_bytes(g) * (size_t)psf_chunk_steps(g);
         p.fixed = align256(sizeof(float) * g->sci.src.size() * (size_t)g->psf_fft * g->psf_fft);
         stage_elems = (size_t)g->sci.stage_elems;
     }
@@ -206,8 +206,12 @@ static int run_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_
             AO_CUDA(launch_trace(g, g->sci, false, g->sci.stage_elems, step0 + c0, ks, dt, v.stage, st), "trace");
             ph = v.stage; api = false; stride = g->sci.stage_elems;
         }
-        for (int k = 0; k < ks; ++k)
-            AO_CUDA(launch_psf(g, ph, api, stride, k, v.scratch, psf, (accumulate || c0 + k > 0) ? 1 : 0, st), "psf");
+        const int kc = psf_chunk_steps(g);
+        for (int k = 0; k < ks; k += kc) {
+            const int kn = ks - k < kc ? ks - k : kc;
+            AO_CUDA(launch_psf(g, ph + (size_t)k * stride, api, stride, kn, v.scratch, psf,
+                               (accumulate || c0 + k > 0) ? 1 : 0, st), "psf");
+        }
     }
     return AO_OK;
 }
@@ -338,6 +342,9 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
                 pr[a] = make_float2((float)cos(PI * (double)q / w.M), (float)sin(PI * (double)q / w.M));
             }
             if ((e = upload(&w.d_tw, t.data(), t.size())) != cudaSuccess) return bail("twiddle upload");
+            std::vector<float2> tf(w.M);
+            for (int k = 0; k < w.M; ++k) tf[k] = make_float2((float)cos(2 * PI * k / w.M), (float)(-sin(2 * PI * k / w.M)));
+            if ((e = upload(&w.d_twf, tf.data(), tf.size())) != cudaSuccess) return bail("twiddle upload");
             if ((e = upload(&w.d_pre, pr.data(), pr.size())) != cudaSuccess) return bail("pre-twiddle upload");
         }
     }
@@ -367,8 +374,8 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
     g->psf_fft = psf_fft;
     if (psf_fft) {
         g->psf_log = ilog2(psf_fft);
-        std::vector<float2> t(psf_fft / 2), pr(g->Np);
-        for (int k = 0; k < psf_fft / 2; ++k) t[k] = make_float2((float)cos(2 * PI * k / psf_fft), (float)(-sin(2 * PI * k / psf_fft)));
+        std::vector<float2> t(psf_fft), pr(g->Np);
+        for (int k = 0; k < psf_fft; ++k) t[k] = make_float2((float)cos(2 * PI * k / psf_fft), (float)(-sin(2 * PI * k / psf_fft)));
         for (int a = 0; a < g->Np; ++a) pr[a] = make_float2((a & 1) ? -1.0f : 1.0f, 0.0f);
         if ((e = upload(&g->d_psf_tw, t.data(), t.size())) != cudaSuccess) return bail("psf twiddle upload");
         if ((e = upload(&g->d_psf_pre, pr.data(), pr.size())) != cudaSuccess) return bail("psf pre upload");

@@ -59,7 +59,8 @@ struct WfsH {
     std::vector<uint8_t> valid;
     int n_valid = 0;
     float2* d_w2m = nullptr;        // W[q] = exp(-i pi q / M), q < 2M     (small path)
-    float2* d_tw = nullptr;         // exp(-2 pi i k / M), k < M/2         (big path)
+    float2* d_tw = nullptr;         // exp(-2 pi i k / M), k < M/2         (big path, generic fallback)
+    float2* d_twf = nullptr;        // exp(-2 pi i k / M), k < M           (big path, Stockham passes)
     float2* d_pre = nullptr;        // pre-twiddle exp(+i pi (M-1) a / M), a < n  (big path)
     void* fused_items = nullptr;    // device WorkItem[]: runs of <= fused_G adjacent valid subapertures
     int n_fused_items = 0, fused_G = 0, fused_R2 = 0;
@@ -80,7 +81,7 @@ struct ao_geometry {
     ao::SourceP* d_sources = nullptr;
     double lambda_ref = 0;
     int psf_fft = 0, psf_log = 0;
-    float2* d_psf_tw = nullptr;
+    float2* d_psf_tw = nullptr;       // exp(-2 pi i k / M), k < M
     float2* d_psf_pre = nullptr;      // (-1)^a as a complex table, a < Np
     ao::Group all, sci;
     long long phase_elems_per_step = 0;
@@ -108,13 +109,14 @@ cudaError_t launch_centroids(ao_geometry* g, const WfsH& w, const float* images,
 cudaError_t launch_noise(ao_geometry* g, const WfsH& w, float* images, int64_t step0, int n_steps,
                          const NoiseP& noise, cudaStream_t st);
 
-// big FFT: SH mode for one step-chunk of WFS w (images out), PSF mode for one step (psf +=).
+// big FFT: SH mode for one step-chunk of WFS w (images out); PSF mode for ks <= psf_chunk_steps(g)
+// consecutive steps summed into psf (phase of step j at phase + j * step_stride).
 cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, bool api_layout,
                           long long step_stride, int n_steps, float2* scratch, float* images,
                           cudaStream_t st);
 cudaError_t launch_psf(ao_geometry* g, const float* phase, bool api_layout, long long step_stride,
-                       int step_in_chunk, float2* scratch, float* psf, int accumulate,
-                       cudaStream_t st);
+                       int ks, float2* scratch, float* psf, int accumulate, cudaStream_t st);
+int psf_chunk_steps(const ao_geometry* g);
 
 // fused trace + SH + CoG (k_fused.cu); cudaErrorNotSupported if the geometry is outside its fast path
 bool fused_supported(const ao_geometry* g, const WfsH& w);
@@ -126,7 +128,7 @@ cudaError_t launch_trace_tiled(ao_geometry* g, const Group& grp, bool api_layout
                                int64_t step0, int n_steps, double dt, float* phase, cudaStream_t st);
 
 size_t sh_big_scratch_bytes(const ao_geometry* g, const WfsH& w);   // per step
-size_t psf_scratch_bytes(const ao_geometry* g);                      // per step
+size_t psf_scratch_bytes(const ao_geometry* g);                      // per step (x psf_chunk_steps)
 
 void set_error(const std::string& msg);
 

@@ -1,128 +1,221 @@
-// k_fft_big.cu -- two-pass HBM FFT for the large transforms (section 2.8 science PSF,
-// reading O7; NGS low-order Shack-Hartmann with M = 1024, readings O3/O4).
+// k_fft_big.cu -- two-pass HBM/L2 FFT for the large transforms: the science PSF (section 2.8,
+// reading O7) and the NGS low-order Shack-Hartmann sensors with FFT > 64 (readings O3/O4).
 //
-// Pass 1 (k_big_rows): one CTA per non-zero input row.  Builds E = A exp(i phi) * pre[a] pre[b]
-//   (pre carries the centring: (-1)^a for the pixel-centred PSF, exp(+i pi (M-1) a/M) for the
-//   half-pixel-centred SH), zero-pads to M in shared memory, runs an in-place radix-2 DIF FFT
-//   and writes the row, in natural order, to the scratch T[batch][a][m].  Rows a >= n are zero
-//   and are never computed or stored (pruning).
-// Pass 2 (k_big_cols): one CTA per group of C adjacent columns.  Loads T[.][a < n][m0..m0+C),
-//   zero-pads, FFTs each column in shared memory, takes |.|^2 * norm and either
-//   accumulates into the PSF (C = 8, 32-byte row segments) or, for the SH, sums the beta x beta
-//   blocks (C = beta: one detector column per CTA; only the detector window is computed).
-// The scratch of one PSF (15.7 MB at 960 x 2048) stays L2-resident between the two passes.
+// Both passes run register-resident Stockham FFTs: a thread holds 16 complex points, a transform of
+// M = 2^LOGM points is T = M/16 threads and two or three radix-16/16/(M/256) passes; points change hands
+// between passes through shared memory padded by one slot every 16 (conflict-free reads and writes);
+// the first pass reads global memory directly and the last one writes it, in natural order.
+//
+// Pass 1 (k_big_rows): the n non-zero input rows only (pruning).  Builds E = A exp(i phi) pre[a] pre[b]
+//   on the fly (pre carries the centring: (-1)^a for the pixel-centred PSF, exp(+i pi (M-1) a/M) for the
+//   half-pixel-centred SH), transforms the zero-padded row and writes it to the scratch T[batch][a][m].
+//   A CTA of 256 threads handles 256/T rows.
+// Pass 2 (k_big_cols): a CTA of T*C threads transforms C adjacent columns (thread = (point group, column),
+//   column fastest, so that global reads are C*8-byte row segments and the shared-memory image is
+//   column-interleaved), takes |.|^2 and
+//   - PSF: accumulates the steps of a chunk in registers and adds them to the long exposure once;
+//   - SH: sums the beta x beta detector bins (C = beta: one detector column per CTA).
+// The scratch of a chunk stays L2-resident between the two passes.
 #include "ao_device.cuh"
+#include "fft_reg.cuh"
 
 namespace ao {
 
-// In-place radix-2 decimation-in-frequency FFT of `nfft` interleaved transforms of length M held
-// in shared memory as x[f*M + i].  Natural-order input, bit-reversed output.  tw[k] = exp(-2 pi i k/M).
-__device__ __forceinline__ void fft_dif_smem(float2* x, int M, int logM, int nfft,
-                                             const float2* __restrict__ tw, int tid, int nt)
+template <int LOGM>
+struct BigCfg {
+    static constexpr int M = 1 << LOGM, T = M / 16;
+    static constexpr int R1 = LOGM <= 8 ? M / 16 : 16;     // radix of the second pass
+    static constexpr int R2 = LOGM <= 8 ? 1 : M / 256;     // radix of the third pass (1 = no third pass)
+    static constexpr int PADM = M + M / 16;                // padded transform length in shared memory
+    static_assert(LOGM >= 6 && LOGM <= 12, "big FFT sizes are 64 .. 4096");
+};
+
+__device__ __forceinline__ float2 cmulf(const float2 a, const float2 b)
 {
-    const int halfM = M >> 1, total = nfft * halfM;
-    for (int s = 0; s < logM; ++s) {
-        const int half = halfM >> s;                 // M/2, M/4, ..., 1
-        for (int t = tid; t < total; t += nt) {
-            const int f = t / halfM, b = t - f * halfM;
-            const int pos = b & (half - 1), grp = b >> (logM - 1 - s);
-            const int i = f * M + grp * 2 * half + pos;
-            const float2 a = x[i], c = x[i + half];
-            const float2 w = __ldg(tw + (pos << s));
-            const float dr = a.x - c.x, di = a.y - c.y;
-            x[i] = make_float2(a.x + c.x, a.y + c.y);
-            x[i + half] = make_float2(dr * w.x - di * w.y, dr * w.y + di * w.x);
+    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+
+// Stockham pass, load half: butterfly b = tb + q T (q < 16/R) reads points b + k M/R, k < R.
+template <int LOGM, int R, typename Load>
+__device__ __forceinline__ void pass_load(const int tb, float2 (&v)[16], Load&& ld)
+{
+    constexpr int M = 1 << LOGM, T = M / 16, Q = 16 / R, STR = M / R;
+#pragma unroll
+    for (int q = 0; q < Q; ++q)
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[q * R + k] = ld(tb + q * T + k * STR);
+}
+
+// Stockham pass, compute half: twiddle exp(-2 pi i (b mod NS) k / (NS R)), R-point DFT, and hand point k of
+// butterfly b to st(index (b / NS) NS R + b mod NS + k NS, value, register slot).
+template <int LOGM, int R, int NS, typename Store>
+__device__ __forceinline__ void pass_compute(const int tb, float2 (&v)[16], const float2* __restrict__ tw, Store&& st)
+{
+    constexpr int M = 1 << LOGM, T = M / 16, Q = 16 / R;
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+        const int b = tb + q * T;
+        float2 x[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) x[k] = v[q * R + k];
+        if constexpr (NS > 1) {
+            const int t0 = (b & (NS - 1)) * (M / (NS * R));
+#pragma unroll
+            for (int k = 1; k < R; ++k) x[k] = cmulf(x[k], __ldg(tw + t0 * k));
         }
-        __syncthreads();
+        if constexpr (R > 1) fft_stage<R, R / 2>(x);
+        const int o = (b / NS) * (NS * R) + (b & (NS - 1));
+#pragma unroll
+        for (int k = 0; k < R; ++k) st(o + k * NS, x[bitrev_c(k, R)], q * R + k);
     }
 }
 
-__global__ void __launch_bounds__(256)
-k_big_rows(const float* __restrict__ phase, long long step_stride, const long long* __restrict__ off,
-           int n_sel, const float* __restrict__ amp, const uint8_t* __restrict__ valid, int n_sub, int n,
-           int M, int logM, const float2* __restrict__ tw, const float2* __restrict__ pre,
-           float2* __restrict__ T)
+// One M-point forward FFT per T threads (tb = index of the thread inside its transform).  Points live in
+// shared memory at sm[(i + i/16) cs + coff].  first(i) supplies input point i, last(i, value, slot) receives
+// output point i (natural order; slot < 16 is a compile-time register index).  Every thread of the CTA must
+// call it (it contains __syncthreads()).
+template <int LOGM, typename First, typename Last>
+__device__ __forceinline__ void big_fft(const int tb, float2* sm, const int cs, const int coff,
+                                        const float2* __restrict__ tw, First&& first, Last&& last)
 {
+    using K = BigCfg<LOGM>;
+    float2 v[16];
+    auto sidx = [&](int i) { return (i + (i >> 4)) * cs + coff; };
+    auto to_smem = [&](int i, const float2 x, int) { sm[sidx(i)] = x; };
+    auto from_smem = [&](int i) { return sm[sidx(i)]; };
+    pass_load<LOGM, 16>(tb, v, first);
+    pass_compute<LOGM, 16, 1>(tb, v, tw, to_smem);
+    __syncthreads();
+    pass_load<LOGM, K::R1>(tb, v, from_smem);
+    if constexpr (K::R2 == 1) {
+        pass_compute<LOGM, K::R1, 16>(tb, v, tw, last);
+    } else {
+        __syncthreads();
+        pass_compute<LOGM, K::R1, 16>(tb, v, tw, to_smem);
+        __syncthreads();
+        pass_load<LOGM, K::R2>(tb, v, from_smem);
+        pass_compute<LOGM, K::R2, 256>(tb, v, tw, last);
+    }
+}
+
+struct BigRowArgs {
+    const float* phase; long long step_stride; const long long* off; int n_sel;
+    const float* amp; const uint8_t* valid; int n_sub, n;
+    const float2* tw; const float2* pre; float2* T;
+};
+
+// Pass 1.  grid (ceil(n / rows per CTA), batch), batch index b = (step * n_sel + si) * n_sub^2 + sa.
+template <int LOGM>
+__global__ void __launch_bounds__(256)
+k_big_rows(const BigRowArgs A)
+{
+    using K = BigCfg<LOGM>;
+    constexpr int M = K::M, T = K::T, RPC = 256 / T;
     extern __shared__ float4 smem_raw[];
-    float2* x = reinterpret_cast<float2*>(smem_raw);
-    const int a = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
-    const int nsa = n_sub * n_sub;
+    float2* sm = reinterpret_cast<float2*>(smem_raw);
+    const int tid = threadIdx.x, r = tid / T, tb = tid - r * T;
+    const int n = A.n, nsa = A.n_sub * A.n_sub;
     const long long b = blockIdx.y;
     const int sa = (int)(b % nsa);
     const long long set = b / nsa;
-    const int si = (int)(set % n_sel);
-    const long long k = set / n_sel;
-    if (valid && !valid[sa]) return;
-    const int p = sa / n_sub, q = sa - p * n_sub, N = n_sub * n;
-    const float* ph = phase + (size_t)k * step_stride + off[si] + (size_t)(p * n + a) * N + q * n;
-    const float* am = amp + (size_t)(p * n + a) * N + q * n;
-    const float2 pa = pre[a];
-    for (int i = tid; i < M; i += nt) {
-        float2 v = make_float2(0.0f, 0.0f);
-        if (i < n) {
-            const float A = am[i];
-            float s, c;
-            sincosf(ph[i], &s, &c);
-            const float2 pb = pre[i];
-            const float wr = pa.x * pb.x - pa.y * pb.y, wi = pa.x * pb.y + pa.y * pb.x;
-            v = make_float2(A * (c * wr - s * wi), A * (c * wi + s * wr));
-        }
-        x[i] = v;
-    }
-    __syncthreads();
-    fft_dif_smem(x, M, logM, 1, tw, tid, nt);
-    float2* out = T + ((size_t)b * n + a) * M;
-    for (int m = tid; m < M; m += nt) out[m] = x[__brev((unsigned)m) >> (32 - logM)];
+    const int si = (int)(set % A.n_sel);
+    const long long k = set / A.n_sel;
+    if (A.valid && !A.valid[sa]) return;                                   // CTA-uniform
+    const int a = blockIdx.x * RPC + r;
+    const bool row_on = a < n;
+    const int p = sa / A.n_sub, q = sa - p * A.n_sub, N = A.n_sub * n;
+    const size_t rowoff = (size_t)(p * n + (row_on ? a : 0)) * N + (size_t)q * n;
+    const float* ph = A.phase + (size_t)k * A.step_stride + A.off[si] + rowoff;
+    const float* am = A.amp + rowoff;
+    const float2 pa = row_on ? A.pre[a] : make_float2(0.0f, 0.0f);
+    float2* out = A.T + ((size_t)b * n + (row_on ? a : 0)) * M;
+    big_fft<LOGM>(tb, sm, 1, r * K::PADM, A.tw,
+        [&](int i) {
+            float2 v = make_float2(0.0f, 0.0f);
+            if (row_on && i < n) {
+                const float Am = __ldg(am + i);
+                float s, c;
+                sincosf(__ldg(ph + i), &s, &c);
+                const float2 w = cmulf(pa, __ldg(A.pre + i));
+                v = cmulf(make_float2(Am * c, Am * s), w);
+            }
+            return v;
+        },
+        [&](int i, const float2 x, int) { if (row_on) out[i] = x; });
 }
 
-// mode 0: PSF (out[dir][k][m] (+)= I), mode 1: SH (images[b][r][g] = binned I)
-template <int MODE>
-__global__ void __launch_bounds__(256)
-k_big_cols(const float2* __restrict__ T, const uint8_t* __restrict__ valid, int nsa, int n, int M, int logM,
-           int C, const float2* __restrict__ tw, float norm, int beta, int P, int k0, int accumulate,
-           float* __restrict__ out)
+struct BigColArgs {
+    const float2* T; const uint8_t* valid; int nsa, n, C;
+    const float2* tw; float norm;
+    int beta, P, k0;                  // SH: detector window
+    int n_dir, ks, accumulate;        // PSF: directions, steps in the chunk, += or =
+    float* out;
+};
+
+// Pass 2.  MODE 0 (PSF): grid (M / C, n_dir); the CTA loops over the ks steps of the chunk.
+//          MODE 1 (SH):  grid (P, batch), C = beta, columns k0 + g beta .. of the detector window.
+template <int LOGM, int MODE>
+__global__ void __launch_bounds__(MODE == 0 ? 512 : 1024)
+k_big_cols(const BigColArgs A)
 {
+    using K = BigCfg<LOGM>;
+    constexpr int M = K::M;
     extern __shared__ float4 smem_raw[];
-    float2* x = reinterpret_cast<float2*>(smem_raw);            // [C][M]
-    const int tid = threadIdx.x, nt = blockDim.x;
+    float2* sm = reinterpret_cast<float2*>(smem_raw);
+    const int tid = threadIdx.x, C = A.C, tb = tid / C, c = tid - tb * C;
+    const int n = A.n, g = blockIdx.x;
     const long long b = blockIdx.y;
-    const int g = blockIdx.x;
-    const int m0 = (MODE == 0) ? g * C : k0 + g * beta;
-    if (MODE == 1 && valid && !valid[(int)(b % nsa)]) {
-        for (int r = tid; r < P; r += nt) out[((size_t)b * P + r) * P + g] = 0.0f;
-        return;
-    }
-    const float2* Tb = T + (size_t)b * n * M;
-    for (int i = tid; i < C * M; i += nt) {
-        const int a = i / C, c = i - a * C;                     // c fastest: C*8-byte segments
-        x[c * M + a] = (a < n) ? Tb[(size_t)a * M + m0 + c] : make_float2(0.0f, 0.0f);
-    }
-    __syncthreads();
-    fft_dif_smem(x, M, logM, C, tw, tid, nt);
     if (MODE == 0) {
-        float* o = out + (size_t)b * M * M;
-        for (int i = tid; i < C * M; i += nt) {
-            const int k = i / C, c = i - k * C;
-            const float2 v = x[c * M + (__brev((unsigned)k) >> (32 - logM))];
-            const float I = (v.x * v.x + v.y * v.y) * norm;
-            const size_t gi = (size_t)k * M + m0 + c;
-            o[gi] = accumulate ? o[gi] + I : I;
+        const int m0 = g * C;
+        float acc[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) acc[i] = 0.0f;
+        for (int k = 0; k < A.ks; ++k) {
+            const float2* Tb = A.T + ((size_t)(k * A.n_dir + b) * n) * M + m0 + c;
+            big_fft<LOGM>(tb, sm, C, c, A.tw,
+                [&](int i) { return i < n ? __ldg(Tb + (size_t)i * M) : make_float2(0.0f, 0.0f); },
+                [&](int, const float2 x, int slot) { acc[slot] = fmaf(x.x, x.x, fmaf(x.y, x.y, acc[slot])); });
+            __syncthreads();                                  // the next step overwrites the exchange buffer
+        }
+        float* o = A.out + (size_t)b * M * M + m0 + c;
+        // replay the index arithmetic of the last pass to place the 16 accumulators
+        constexpr int RL = K::R2 == 1 ? K::R1 : K::R2, NSL = K::R2 == 1 ? 16 : 256, Q = 16 / RL;
+#pragma unroll
+        for (int q = 0; q < Q; ++q) {
+            const int bb = tb + q * K::T;
+            const int o0 = (bb / NSL) * (NSL * RL) + (bb & (NSL - 1));
+#pragma unroll
+            for (int kk = 0; kk < RL; ++kk) {
+                const size_t gi = (size_t)(o0 + kk * NSL) * M;
+                const float I = acc[q * RL + kk] * A.norm;
+                o[gi] = A.accumulate ? o[gi] + I : I;
+            }
         }
     } else {
-        for (int r = tid; r < P; r += nt) {
-            float s = 0.0f;
-            for (int kk = 0; kk < beta; ++kk) {
-                const int kr = __brev((unsigned)(k0 + r * beta + kk)) >> (32 - logM);
-                for (int c = 0; c < beta; ++c) {
-                    const float2 v = x[c * M + kr];
-                    s += (v.x * v.x + v.y * v.y) * norm;
-                }
-            }
-            out[((size_t)b * P + r) * P + g] = s;
+        __shared__ float pix[1024];
+        const int sa = (int)(b % A.nsa);
+        if (A.valid && !A.valid[sa]) {
+            for (int r = tid; r < A.P; r += blockDim.x) A.out[((size_t)b * A.P + r) * A.P + g] = 0.0f;
+            return;
         }
+        for (int r = tid; r < A.P; r += blockDim.x) pix[r] = 0.0f;
+        __syncthreads();
+        const int m0 = A.k0 + g * A.beta;
+        const float2* Tb = A.T + (size_t)b * n * M + m0 + c;
+        const int kend = A.k0 + A.beta * A.P;
+        big_fft<LOGM>(tb, sm, C, c, A.tw,
+            [&](int i) { return i < n ? __ldg(Tb + (size_t)i * M) : make_float2(0.0f, 0.0f); },
+            [&](int i, const float2 x, int) {
+                float I = fmaf(x.x, x.x, x.y * x.y);
+                for (int o = 1; o < C; o <<= 1) I += __shfl_xor_sync(0xffffffffu, I, o);   // the beta columns
+                if (c == 0 && i >= A.k0 && i < kend) atomicAdd(&pix[(i - A.k0) / A.beta], I);
+            });
+        __syncthreads();
+        for (int r = tid; r < A.P; r += blockDim.x) A.out[((size_t)b * A.P + r) * A.P + g] = pix[r] * A.norm;
     }
 }
 
+// ---- host side -------------------------------------------------------------------------------
 size_t sh_big_scratch_bytes(const ao_geometry*, const WfsH& w)
 {
     return sizeof(float2) * (size_t)w.grp.src.size() * w.n_sub * w.n_sub * w.n * w.M;
@@ -133,59 +226,139 @@ size_t psf_scratch_bytes(const ao_geometry* g)
     return sizeof(float2) * g->sci.src.size() * (size_t)g->Np * g->psf_fft;
 }
 
+// Steps of the science PSF transformed per launch pair: the column pass sums them in registers, so the
+// long exposure is read and written once per chunk; the scratch of a chunk should stay inside L2.
+int psf_chunk_steps(const ao_geometry* g)
+{
+    const size_t per = psf_scratch_bytes(g);
+    if (per == 0) return 1;
+    const size_t budget = (size_t)64 << 20;
+    size_t ks = budget / per;
+    if (ks < 1) ks = 1;
+    if (ks > 8) ks = 8;
+    return (int)ks;
+}
+
+static int cols_threads_per_transform(int M) { return M / 16; }
+
+// The SH fast path needs C = beta columns per CTA: a power of two, full warps, at most 1024 threads.
+bool sh_big_fast(const WfsH& w)
+{
+    if (w.M < 128 || w.M > 4096 || (w.M & (w.M - 1))) return false;
+    const int T = cols_threads_per_transform(w.M), C = w.beta;
+    if (C < 1 || C > 32 || (C & (C - 1))) return false;
+    if (T * C < 32 || T * C > 1024 || w.P > 1024) return false;
+    return sizeof(float2) * (size_t)C * (w.M + w.M / 16) <= 200 * 1024;
+}
+
+template <int LOGM>
+static cudaError_t launch_rows_t(const BigRowArgs& a, int n_rows, unsigned batch, cudaStream_t st)
+{
+    using K = BigCfg<LOGM>;
+    constexpr int RPC = 256 / K::T;
+    const size_t smem = sizeof(float2) * (size_t)RPC * K::PADM;
+    cudaError_t e = cudaFuncSetAttribute(k_big_rows<LOGM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_big_rows<LOGM><<<dim3((n_rows + RPC - 1) / RPC, batch), 256, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <int LOGM, int MODE>
+static cudaError_t launch_cols_t(const BigColArgs& a, unsigned gx, unsigned gy, cudaStream_t st)
+{
+    using K = BigCfg<LOGM>;
+    const size_t smem = sizeof(float2) * (size_t)a.C * K::PADM;
+    cudaError_t e = cudaFuncSetAttribute(k_big_cols<LOGM, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_big_cols<LOGM, MODE><<<dim3(gx, gy), K::T * a.C, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+#define AO_BIG_DISPATCH(logM, CALL)                                   \
+    switch (logM) {                                                   \
+        case 6: { constexpr int L = 6; return CALL; }                 \
+        case 7: { constexpr int L = 7; return CALL; }                 \
+        case 8: { constexpr int L = 8; return CALL; }                 \
+        case 9: { constexpr int L = 9; return CALL; }                 \
+        case 10: { constexpr int L = 10; return CALL; }               \
+        case 11: { constexpr int L = 11; return CALL; }               \
+        case 12: { constexpr int L = 12; return CALL; }               \
+        default: return cudaErrorNotSupported;                        \
+    }
+
+static cudaError_t launch_rows(int logM, const BigRowArgs& a, int n_rows, unsigned batch, cudaStream_t st)
+{
+    AO_BIG_DISPATCH(logM, launch_rows_t<L>(a, n_rows, batch, st))
+}
+static cudaError_t launch_cols_psf(int logM, const BigColArgs& a, unsigned gx, unsigned gy, cudaStream_t st)
+{
+    AO_BIG_DISPATCH(logM, (launch_cols_t<L, 0>(a, gx, gy, st)))
+}
+static cudaError_t launch_cols_sh(int logM, const BigColArgs& a, unsigned gx, unsigned gy, cudaStream_t st)
+{
+    AO_BIG_DISPATCH(logM, (launch_cols_t<L, 1>(a, gx, gy, st)))
+}
+
+cudaError_t launch_sh_big_generic(ao_geometry* g, const WfsH& w, const float* phase, bool api_layout,
+                                  long long step_stride, int n_steps, float2* scratch, float* images,
+                                  cudaStream_t st);
+
 cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, bool api_layout,
                           long long step_stride, int n_steps, float2* scratch, float* images,
                           cudaStream_t st)
 {
+    if (!sh_big_fast(w)) return launch_sh_big_generic(g, w, phase, api_layout, step_stride, n_steps, scratch, images, st);
     const int n_sel = (int)w.grp.src.size(), nsa = w.n_sub * w.n_sub;
     if (n_sel == 0 || n_steps <= 0) return cudaSuccess;
     cudaError_t e;
-    const size_t smem_r = sizeof(float2) * w.M, smem_c = sizeof(float2) * (size_t)w.beta * w.M;
-    e = cudaFuncSetAttribute(k_big_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_r);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_big_cols<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c);
-    if (e != cudaSuccess) return e;
-    const float norm = (float)(1.0 / ((double)w.M * w.M * (double)w.n * w.n));
-    const int k0 = (w.M - w.beta * w.P) / 2;
+    const unsigned batch = (unsigned)(n_sel * nsa);
     // one step at a time: the scratch holds one step of this WFS
     for (int k = 0; k < n_steps; ++k) {
-        const unsigned batch = (unsigned)(n_sel * nsa);
-        k_big_rows<<<dim3(w.n, batch), 256, smem_r, st>>>(
-            phase + (size_t)k * step_stride, step_stride, api_layout ? w.grp.d_off_api : w.grp.d_off_stage,
-            n_sel, w.d_amp, w.d_valid, w.n_sub, w.n, w.M, w.logM, w.d_tw, w.d_pre, scratch);
+        BigRowArgs r;
+        r.phase = phase + (size_t)k * step_stride; r.step_stride = step_stride;
+        r.off = api_layout ? w.grp.d_off_api : w.grp.d_off_stage; r.n_sel = n_sel;
+        r.amp = w.d_amp; r.valid = w.d_valid; r.n_sub = w.n_sub; r.n = w.n;
+        r.tw = w.d_twf; r.pre = w.d_pre; r.T = scratch;
+        if ((e = launch_rows(w.logM, r, w.n, batch, st)) != cudaSuccess) return e;
         g->launches++;
-        if ((e = cudaGetLastError()) != cudaSuccess) return e;
-        k_big_cols<1><<<dim3(w.P, batch), 256, smem_c, st>>>(
-            scratch, w.d_valid, nsa, w.n, w.M, w.logM, w.beta, w.d_tw, norm, w.beta, w.P, k0, 0,
-            images + (size_t)k * batch * w.P * w.P);
+        BigColArgs c;
+        c.T = scratch; c.valid = w.d_valid; c.nsa = nsa; c.n = w.n; c.C = w.beta; c.tw = w.d_twf;
+        c.norm = (float)(1.0 / ((double)w.M * w.M * (double)w.n * w.n));
+        c.beta = w.beta; c.P = w.P; c.k0 = (w.M - w.beta * w.P) / 2;
+        c.n_dir = 1; c.ks = 1; c.accumulate = 0;
+        c.out = images + (size_t)k * batch * w.P * w.P;
+        if ((e = launch_cols_sh(w.logM, c, (unsigned)w.P, batch, st)) != cudaSuccess) return e;
         g->launches++;
-        if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
     return cudaSuccess;
 }
 
+// Science PSF of `ks` consecutive steps (phase of step j at phase + j * step_stride), summed and then
+// added to (accumulate != 0) or stored in psf.  ks <= psf_chunk_steps(g): the scratch holds ks steps.
 cudaError_t launch_psf(ao_geometry* g, const float* phase, bool api_layout, long long step_stride,
-                       int step_in_chunk, float2* scratch, float* psf, int accumulate, cudaStream_t st)
+                       int ks, float2* scratch, float* psf, int accumulate, cudaStream_t st)
 {
-    const int n_dir = (int)g->sci.src.size(), M = g->psf_fft, C = 8;
-    if (n_dir == 0) return cudaSuccess;
+    const int n_dir = (int)g->sci.src.size(), M = g->psf_fft;
+    if (n_dir == 0 || ks <= 0) return cudaSuccess;
     cudaError_t e;
-    const size_t smem_r = sizeof(float2) * M, smem_c = sizeof(float2) * (size_t)C * M;
-    e = cudaFuncSetAttribute(k_big_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_r);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_big_cols<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c);
-    if (e != cudaSuccess) return e;
-    const float norm = g->sumA2 > 0 ? (float)(1.0 / ((double)M * M * g->sumA2)) : 0.0f;
-    k_big_rows<<<dim3(g->Np, n_dir), 256, smem_r, st>>>(
-        phase + (size_t)step_in_chunk * step_stride, step_stride,
-        api_layout ? g->sci.d_off_api : g->sci.d_off_stage, n_dir, g->d_pupil_amp, nullptr, 1, g->Np, M,
-        g->psf_log, g->d_psf_tw, g->d_psf_pre, scratch);
+    BigRowArgs r;
+    r.phase = phase; r.step_stride = step_stride;
+    r.off = api_layout ? g->sci.d_off_api : g->sci.d_off_stage; r.n_sel = n_dir;
+    r.amp = g->d_pupil_amp; r.valid = nullptr; r.n_sub = 1; r.n = g->Np;
+    r.tw = g->d_psf_tw; r.pre = g->d_psf_pre; r.T = scratch;
+    if ((e = launch_rows(g->psf_log, r, g->Np, (unsigned)(ks * n_dir), st)) != cudaSuccess) return e;
     g->launches++;
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    k_big_cols<0><<<dim3(M / C, n_dir), 256, smem_c, st>>>(scratch, nullptr, 1, g->Np, M, g->psf_log, C,
-                                                         g->d_psf_tw, norm, 1, 1, 0, accumulate, psf);
+    const int T = cols_threads_per_transform(M);
+    int C = 4;
+    while (T * C < 128) C *= 2;                              // small transforms: keep at least 4 warps per CTA
+    while (T * C > 512) C /= 2;                              // launch bound of the PSF column pass
+    BigColArgs c;
+    c.T = scratch; c.valid = nullptr; c.nsa = 1; c.n = g->Np; c.C = C; c.tw = g->d_psf_tw;
+    c.norm = g->sumA2 > 0 ? (float)(1.0 / ((double)M * M * g->sumA2)) : 0.0f;
+    c.beta = 1; c.P = 1; c.k0 = 0; c.n_dir = n_dir; c.ks = ks; c.accumulate = accumulate; c.out = psf;
+    if ((e = launch_cols_psf(g->psf_log, c, (unsigned)(M / C), (unsigned)n_dir, st)) != cudaSuccess) return e;
     g->launches++;
-    return cudaGetLastError();
+    return cudaSuccess;
 }
 
 }  // namespace ao

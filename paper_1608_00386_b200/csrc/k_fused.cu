@@ -22,78 +22,14 @@
 // noise, centre of gravity by warp shuffles.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <type_traits>
 #include <vector>
 
+#include "fft_reg.cuh"
 #include "trace_tile.cuh"
 
 namespace ao {
-
-// ------------------------------------------------------------------------------------------------
-// compile-time trigonometry and complex constants
-constexpr double kPi = 3.14159265358979323846264338327950288;
-constexpr double cx_sin(double x)
-{
-    double t = x, s = x;
-    for (int i = 1; i < 28; ++i) { t *= -x * x / ((2.0 * i) * (2.0 * i + 1.0)); s += t; }
-    return s;
-}
-constexpr double cx_cos(double x)
-{
-    double t = 1.0, s = 1.0;
-    for (int i = 1; i < 28; ++i) { t *= -x * x / ((2.0 * i - 1.0) * (2.0 * i)); s += t; }
-    return s;
-}
-
-// cis(pi NUM / DEN) as compile-time floats
-template <int NUM, int DEN>
-struct Cis {
-    static constexpr int q = ((NUM % (2 * DEN)) + 2 * DEN) % (2 * DEN);       // angle = pi q / DEN in [0, 2 pi)
-    static constexpr int qs = q >= DEN ? q - 2 * DEN : q;                      // in [-pi, pi)
-    static constexpr float re = (float)cx_cos(kPi * (double)qs / (double)DEN);
-    static constexpr float im = (float)cx_sin(kPi * (double)qs / (double)DEN);
-};
-
-template <int NUM, int DEN>
-__device__ __forceinline__ float2 cmul_cis(const float2 x)
-{
-    using W = Cis<NUM, DEN>;
-    if constexpr (W::q == 0) return x;
-    else if constexpr (2 * W::q == DEN) return make_float2(-x.y, x.x);
-    else if constexpr (W::q == DEN) return make_float2(-x.x, -x.y);
-    else if constexpr (2 * W::q == 3 * DEN) return make_float2(x.y, -x.x);
-    else return make_float2(fmaf(x.x, W::re, -x.y * W::im), fmaf(x.x, W::im, x.y * W::re));
-}
-
-template <int I, int N, typename F>
-__device__ __forceinline__ void static_for(F&& f)
-{
-    if constexpr (I < N) {
-        f(std::integral_constant<int, I>{});
-        static_for<I + 1, N>(static_cast<F&&>(f));
-    }
-}
-
-__host__ __device__ constexpr int bitrev_c(int k, int n)
-{
-    int r = 0;
-    for (int b = 1; b < n; b <<= 1) { r = (r << 1) | (k & 1); k >>= 1; }
-    return r;
-}
-
-// In-register radix-2 DIF FFT, forward sign, natural-order input, X[k] = x[bitrev(k)] on output.
-template <int N, int HALF>
-__device__ __forceinline__ void fft_stage(float2 (&x)[N])
-{
-    static_for<0, N / 2>([&](auto bi) {
-        constexpr int b = decltype(bi)::value;
-        constexpr int grp = b / HALF, pos = b % HALF, i = grp * 2 * HALF + pos, j = i + HALF;
-        const float2 a = x[i], c = x[j];
-        x[i] = make_float2(a.x + c.x, a.y + c.y);
-        x[j] = cmul_cis<-pos, HALF>(make_float2(a.x - c.x, a.y - c.y));      // * exp(-2 pi i pos/(2 HALF))
-    });
-    if constexpr (HALF > 1) fft_stage<N, HALF / 2>(x);
-}
 
 // Half-pixel-centred DFT of size M = 2n of n inputs (zero padded):
 //   X[k] = sum_a e[a] exp(-2 pi i (k - (M-1)/2) a / M),  k < M.
@@ -350,6 +286,7 @@ static TilePlan plan_tiles(const ao_geometry* g, const std::vector<int>& src, si
     const size_t stage = (size_t)pl.rows * pl.pitch * sizeof(float);
     // 4 CTAs per SM need <= ~48 KB of dynamic shared memory each; prefer 3 stages when they fit
     pl.ns = (3 * stage <= 48 * 1024) ? 3 : 2;
+    if (const char* ev = getenv("AO_FUSED_STAGES")) { const int v = atoi(ev); if (v >= 2 && v <= kTraceMaxStages) pl.ns = v; }
     pl.smem = pl.ns * stage;
     if (pl.smem < min_bytes) pl.smem = min_bytes;
     pl.smem += 128;

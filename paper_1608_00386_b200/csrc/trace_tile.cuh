@@ -85,7 +85,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 
 constexpr int kTraceRows = 32;          // output rows of a tile
-constexpr int kTraceMaxStages = 3;
+constexpr int kTraceMaxStages = 4;
 
 struct TraceArgs {
     const LayerP* layers; int n_layers;

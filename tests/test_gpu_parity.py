@@ -272,3 +272,26 @@ def test_forward_host_matches_device_path():
                 assert np.abs(sl[w][k, si].numpy() - ref["slopes"][s][k]).max() <= SLOPE_TOL
     for di, s in enumerate(cfg.science_sources()):
         assert rel_l2(psf[di].numpy(), ref["psf"][s]) <= IMAGE_TOL
+
+
+@pytest.mark.parametrize("n_sub,psf_fft,n_steps", [(4, 64, 2), (20, None, 10), (40, None, 2), (20, 4096, 1), (80, None, 1)])
+def test_big_fft_sizes_ngs_sensor_and_psf(n_sub, psf_fft, n_steps):
+    """Two-pass register-resident FFT at every pass structure (16x4 .. 16x16x16): NGS sensor with
+    FFT 64..1024 (2x2 subapertures, bin 8) and the science PSF with FFT 64..4096; the PSF long exposure
+    is summed over more steps than one internal chunk holds (n_steps = 10)."""
+    import torch
+    cfg = inputs.make_config(4, n_sub=n_sub, screen_n=1024, n_steps=n_steps, lgs_fft=16, n_layers=2,
+                             psf_fft=psf_fft)
+    srcs = cfg.sources_of_wfs(1) + cfg.science_sources()
+    ref = oracle.forward(cfg, 3, n_steps, want_phase=False, sources=srcs)
+    geo = _geo(cfg, n_steps)
+    img, slp = geo.sh_images(1, None, 3, n_steps, cfg.dt_s)
+    torch.cuda.synchronize()
+    check_wfs(cfg, geo, ref, 1, img, slp, n_steps, f"NGS fft {cfg.wfs[1].fft}")
+    p = geo.psf(None, 3, n_steps, cfg.dt_s)
+    p2 = geo.psf(None, 3, n_steps, cfg.dt_s, psf=p.clone(), accumulate=True)
+    torch.cuda.synchronize()
+    for di, s in enumerate(cfg.science_sources()):
+        assert rel_l2(p[di].cpu().numpy(), ref["psf"][s]) <= IMAGE_TOL
+        assert rel_l2(p2[di].cpu().numpy(), 2.0 * ref["psf"][s]) <= IMAGE_TOL
+        assert abs(float(p[di].sum()) / n_steps - 1.0) < 1e-4          # Parseval: every PSF sums to 1
