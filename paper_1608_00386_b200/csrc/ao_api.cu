@@ -153,7 +153,7 @@ static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0
     const size_t n_sel = w.grp.src.size(), nsa = (size_t)w.n_sub * w.n_sub, PP = (size_t)w.P * w.P;
     if (n_sel == 0) return AO_OK;
     if (!phase_dev && !w.big) {                       // hot path: one fused kernel, no phase in HBM, no workspace
-        if (fused_supported(g, w)) {
+        if (fused_supported(g, w, dt)) {
             AO_CUDA(launch_fused(g, w, step0, n_steps, dt, make_noise(noise), images, slopes, st), "fused");
             return AO_OK;
         }

@@ -119,7 +119,7 @@ cudaError_t launch_psf(ao_geometry* g, const float* phase, bool api_layout, long
 int psf_chunk_steps(const ao_geometry* g);
 
 // fused trace + SH + CoG (k_fused.cu); cudaErrorNotSupported if the geometry is outside its fast path
-bool fused_supported(const ao_geometry* g, const WfsH& w);
+bool fused_supported(const ao_geometry* g, const WfsH& w, double dt);
 cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_steps, double dt,
                          const NoiseP& noise, float* images, float* slopes, cudaStream_t st);
 void fused_tile_shape(int M, int* G, int* R2);

@@ -1,16 +1,15 @@
 // k_fused.cu -- the WFS hot path: ray-trace + Shack-Hartmann image + centre of gravity in ONE kernel
 // (ao_sh_images with phase_dev == NULL for M in {16, 32}, n = M/2, beta*P = M, P = 8; PAPER.md:56,60,28,82;
-// readings O2, O3, O4, O5, O6), and k_trace_tiled, the same tiled ray-trace writing phase to HBM
-// (ao_trace_layers and the internal staging of the big-FFT sensors / science PSF).
+// readings O2, O3, O4, O5, O6).
 //
-// Work decomposition of k_fused.  A CTA (128 threads) processes one work item of one (step, source): a tile
-// of 32 rows x 256 columns of phase samples = R2 = 32/n subaperture rows by up to G = 256/n horizontally
-// adjacent subapertures, built at create time from runs of valid subapertures (invalid ones are never
-// scheduled; their outputs are zero-filled by a memset).  CTAs of consecutive time steps of the same tile
-// are adjacent in the grid (step is the fastest index): their screen footprints differ by a sub-pixel wind
-// shift, so all but the first hit in L2.
+// Work decomposition of k_fused.  A CTA (128 threads) processes one work item of one source for TWO
+// consecutive time steps: a tile of 16 rows x 256 columns of phase samples = R2 = 16/n subaperture rows by up
+// to G = 256/n horizontally adjacent subapertures, built at create time from runs of valid subapertures
+// (invalid ones are never scheduled; their outputs are zero-filled by a memset).  The two steps share one
+// staged screen box per layer (frozen flow: their footprints differ by the wind shift only).  CTAs of
+// consecutive step pairs of the same tile are adjacent in the grid: all but the first hit in L2.
 //
-// Phase A, ray-trace: trace_tile.cuh.  The phase of the tile ends in registers; it never touches HBM.
+// Phase A, ray-trace: trace2.cuh.  The phase of the tile ends in registers; it never touches HBM.
 //
 // Phase B, image formation, one round per (subaperture row, column slot); the rounds are a rolled loop so
 // that the FFT code exists once (instruction cache).  Thread (g, b) holds column b of subaperture g of the
@@ -27,7 +26,7 @@
 #include <vector>
 
 #include "fft_reg.cuh"
-#include "trace_tile.cuh"
+#include "trace2.cuh"
 
 namespace ao {
 
@@ -52,10 +51,10 @@ __device__ __forceinline__ void dft_half_padded(const float2 (&e)[M / 2], Sink&&
 struct WorkItem { int p, q0, cnt, pad; };
 
 struct FusedArgs {
-    TraceArgs T;
+    Trace2Args T;
     const int* sel; int n_sel;
     const WorkItem* items; int n_items;
-    int n_steps;
+    int n_steps, n_pairs;
     const float* amp;                 // [N][N] on the WFS grid
     const uint8_t* valid;             // [n_sub^2]
     int n_sub;
@@ -72,15 +71,16 @@ template <int M>
 struct FusedCfg {
     static constexpr int n = M / 2;
     static constexpr int NT = kFusedThreads;
-    static constexpr int R2 = kTraceRows / n;            // subaperture rows per tile
+    static constexpr int R2 = kTR / n;                   // subaperture rows per tile
     static constexpr int G = kTileCols / n;              // subapertures per tile row
     static constexpr int GS = NT / n;                    // subapertures per round
-    static constexpr int ROUNDS = 2 * R2;
+    static constexpr int HS = kKS * R2;                  // (step, subaperture row) slices held in registers
+    static constexpr int ROUNDS = 2 * HS;
     static constexpr int P = 8, BETA = M / 8;
     static constexpr int XP = n + 1;                     // transpose pitch (float2 units)
     static constexpr int SUB_STRIDE = M * XP + (n == 8 ? 8 : 0);
     static constexpr size_t XCH_BYTES = (size_t)GS * SUB_STRIDE * sizeof(float2);
-    static_assert(kTraceRows % n == 0 && NT % n == 0 && n <= 32, "bad fused configuration");
+    static_assert(kTR % n == 0 && NT % n == 0 && n <= 32, "bad fused configuration");
 };
 
 template <int M, bool NOISE>
@@ -90,36 +90,37 @@ k_fused(const FusedArgs A)
     using K = FusedCfg<M>;
     constexpr int n = K::n, NT = K::NT, R2 = K::R2, P = K::P, BETA = K::BETA;
     extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ TraceShared S;
+    __shared__ Trace2Shared S;
 
     const int tid = threadIdx.x;
-    // step is the fastest block index: consecutive CTAs share their screen footprint through L2
-    const int k = (int)(blockIdx.x % (unsigned)A.n_steps);
-    const unsigned rest = blockIdx.x / (unsigned)A.n_steps;
+    // the step pair is the fastest block index: consecutive CTAs share their screen footprint through L2
+    const int kp = (int)(blockIdx.x % (unsigned)A.n_pairs);
+    const unsigned rest = blockIdx.x / (unsigned)A.n_pairs;
     const WorkItem it = A.items[rest % (unsigned)A.n_items];
     const int si = (int)(rest / (unsigned)A.n_items);
     const int src_index = A.sel[si];
     const SourceP sp = A.T.srcs[src_index];
     const int N = A.n_sub * n, nsa = A.n_sub * A.n_sub;
 
-    // ---- phase A: ray-trace of the 32 x 256 tile into registers ----
-    u64 acc[kTraceRows];
-    double refsum[2];
-    trace_tile<NT, n>(A.T, sp, S, reinterpret_cast<float*>(smem), it.q0 * n, it.p * n, A.T.step0 + k, acc, refsum);
+    // ---- phase A: ray-trace of the 16 x 256 tile, two steps, into registers ----
+    u64 acc[kKS * kTR];
+    trace2_tile<NT>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc);
     __syncthreads();                                       // stages are dead: shared memory becomes the exchange buffer
 
     // ---- phase B: image formation, one (subaperture row, column slot) round at a time ----
     float2* xch = reinterpret_cast<float2*>(smem);
     const float scale = (float)sp.scale;
     const int g = tid / n, b = tid - g * n;                // subaperture in round, column in subaperture
-    const size_t set = (size_t)k * A.n_sel + si;
     float2* xs = xch + (size_t)g * K::SUB_STRIDE;
 #pragma unroll 1
     for (int rd = 0; rd < K::ROUNDS; ++rd) {
-        const int h = rd >> 1, c = rd & 1;
+        const int hs = rd >> 1, c = rd & 1;                // hs = step-in-pair * R2 + subaperture row
+        const int sp2 = hs / R2, h = hs - sp2 * R2;
+        const int k = 2 * kp + sp2;
+        const size_t set = (size_t)k * A.n_sel + si;
         const int gs = c * K::GS + g;                      // subaperture within the item (column c*NT + tid)
         const int q = it.q0 + gs, p = it.p + h;
-        const bool inb = gs < it.cnt && p < A.n_sub;
+        const bool inb = gs < it.cnt && p < A.n_sub && k < A.n_steps;
         const int sa = inb ? p * A.n_sub + q : 0;
         const bool active = inb && A.valid[sa] != 0;
         if (!__any_sync(0xffffffffu, active)) continue;
@@ -131,7 +132,7 @@ k_fused(const FusedArgs A)
             for (int i = 0; i < n; ++i) {
                 u64 v = acc[i];
 #pragma unroll
-                for (int hh = 1; hh < R2; ++hh) v = (h == hh) ? acc[hh * n + i] : v;
+                for (int hh = 1; hh < K::HS; ++hh) v = (hs == hh) ? acc[hh * n + i] : v;
                 const float2 f = unpack2(v);
                 const float ph = (c ? f.y : f.x) * scale;
                 const float Am = active ? __ldg(ap + (size_t)i * N) : 0.0f;
@@ -216,57 +217,18 @@ k_fused(const FusedArgs A)
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_trace_tiled: the same tiled ray-trace, phase written to HBM (absolute: the FP64 piston sum is added back).
-struct TiledTraceArgs {
-    TraceArgs T;
-    const int* sel; const long long* off; int n_sel;
-    long long step_stride;
-    int n_steps, tiles_x, tiles_y;
-    float* phase;
-};
-
-__global__ void __launch_bounds__(kFusedThreads, 4)
-k_trace_tiled(const TiledTraceArgs A)
-{
-    extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ TraceShared S;
-    const int tid = threadIdx.x;
-    const int k = (int)(blockIdx.x % (unsigned)A.n_steps);
-    unsigned rest = blockIdx.x / (unsigned)A.n_steps;
-    const int tx = (int)(rest % (unsigned)A.tiles_x); rest /= (unsigned)A.tiles_x;
-    const int ty = (int)(rest % (unsigned)A.tiles_y);
-    const int si = (int)(rest / (unsigned)A.tiles_y);
-    const SourceP sp = A.T.srcs[A.sel[si]];
-    const int jfirst = tx * kTileCols, ifirst = ty * kTraceRows;
-    if (jfirst >= sp.N || ifirst >= sp.N) return;          // CTA-uniform
-    u64 acc[kTraceRows];
-    double refsum[2];
-    trace_tile<kFusedThreads, 1>(A.T, sp, S, reinterpret_cast<float*>(smem), jfirst, ifirst, A.T.step0 + k, acc, refsum);
-    float* out = A.phase + (size_t)k * A.step_stride + A.off[si];
-    const int j0 = jfirst + tid, j1 = j0 + kFusedThreads;
-#pragma unroll
-    for (int i = 0; i < kTraceRows; ++i) {
-        const int row = ifirst + i;
-        if (row < sp.N) {
-            const float2 f = unpack2(acc[i]);
-            if (j0 < sp.N) out[(size_t)row * sp.N + j0] = (float)(((double)f.x + refsum[0]) * sp.scale);
-            if (j1 < sp.N) out[(size_t)row * sp.N + j1] = (float)(((double)f.y + refsum[1]) * sp.scale);
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
 // host side
 struct TilePlan { bool ok; int pitch, rows, ns; size_t smem; };
 
-// Staging plan of the tiled ray-trace for the sources `src` (all active layers): the box of a 32 x 256 tile
-// must fit the shared-memory stages and the row march needs 0 < du <= 1.  `min_bytes`: floor on the dynamic
-// shared memory (the exchange buffer of k_fused).
-static TilePlan plan_tiles(const ao_geometry* g, const std::vector<int>& src, size_t min_bytes)
+// Staging plan of the two-step tiled ray-trace for the sources `src` (all active layers): the union box of a
+// 16 x 256 tile over two consecutive steps must fit a shared-memory stage and the row march needs
+// 0 < du <= 1.  `min_bytes`: floor on the stage region (the exchange buffer of k_fused aliases it).
+static TilePlan plan_tiles(const ao_geometry* g, const std::vector<int>& src, double dt, size_t min_bytes)
 {
     TilePlan pl = {false, 0, 0, 0, 0};
-    double du_max = 0.0;
+    double ext_x = 0.0, ext_y = 0.0;                               // box extent beyond the taps, screen pixels
     int s_min = 1 << 30;
+    bool any = false;
     for (int s : src) {
         const SourceP& sp = g->sources[s];
         for (const LayerP& lp : g->layers) {
@@ -275,30 +237,38 @@ static TilePlan plan_tiles(const ao_geometry* g, const std::vector<int>& src, si
             if (fabs(du - 1.0) < 1e-9) du = 1.0;
             if (!(du > 0.0) || du > 1.0) return pl;              // the row march assumes 0 < du <= 1
             if (lp.S % 4 != 0) return pl;                          // 16-byte aligned rows for the bulk copies
-            if (du > du_max) du_max = du;
+            const double shx = fabs(lp.wx * dt * lp.inv_pitch) * (kKS - 1), shy = fabs(lp.wy * dt * lp.inv_pitch) * (kKS - 1);
+            ext_x = std::max(ext_x, (kTileCols - 1) * du + shx);
+            ext_y = std::max(ext_y, (kTR - 1) * du + shy);
             if (lp.S < s_min) s_min = lp.S;
+            any = true;
         }
     }
-    if (du_max == 0.0) { du_max = 1.0; s_min = 1 << 30; }          // no active layer at all: any plan works
-    pl.pitch = (((int)ceil((kTileCols - 1) * du_max) + 7) + 3) & ~3;
-    pl.rows = (int)ceil((kTraceRows - 1) * du_max) + 3 + 1;       // box rows + one prefetch pad row
+    if (!any) { ext_x = kTileCols - 1; ext_y = kTR - 1; }
+    if (!(ext_x < 4096.0 && ext_y < 4096.0)) return pl;            // absurd wind shift per step: not this path
+    pl.pitch = (((int)ceil(ext_x) + 8) + 3) & ~3;                  // + alignment (3), right tap, rounding slack
+    pl.rows = (int)ceil(ext_y) + 3 + 1;                            // box rows + one prefetch pad row
     if (s_min < pl.pitch || s_min < pl.rows) return pl;            // a box row may wrap the screen edge once only
     const size_t stage = (size_t)pl.rows * pl.pitch * sizeof(float);
-    // 4 CTAs per SM need <= ~48 KB of dynamic shared memory each; prefer 3 stages when they fit
-    pl.ns = (3 * stage <= 48 * 1024) ? 3 : 2;
-    if (const char* ev = getenv("AO_FUSED_STAGES")) { const int v = atoi(ev); if (v >= 2 && v <= kTraceMaxStages) pl.ns = v; }
-    pl.smem = pl.ns * stage;
-    if (pl.smem < min_bytes) pl.smem = min_bytes;
-    pl.smem += 128;
+    const size_t sched = trace2_sched_bytes((int)g->layers.size());
+    // 4 CTAs per SM: <= ~55 KB of shared memory each; as many stages (<= 4) as fit, at least 2
+    const size_t budget = 55 * 1024 + 512;
+    pl.ns = 2;
+    while (pl.ns < kT2MaxStages && (pl.ns + 1) * stage + sched + 128 + 256 <= budget) ++pl.ns;
+    if (const char* ev = getenv("AO_FUSED_STAGES")) { const int v = atoi(ev); if (v >= 2 && v <= kT2MaxStages) pl.ns = v; }
+    size_t region = pl.ns * stage;
+    if (region < min_bytes) region = (min_bytes + 15) & ~(size_t)15;
+    pl.smem = region + sched + 128;
     pl.ok = pl.smem <= 200 * 1024;
     return pl;
 }
 
-static TraceArgs make_trace_args(const ao_geometry* g, const TilePlan& pl, int64_t step0, double dt)
+static Trace2Args make_trace_args(const ao_geometry* g, const TilePlan& pl, int64_t step0, double dt)
 {
-    TraceArgs t;
+    Trace2Args t;
     t.layers = g->d_layers; t.n_layers = (int)g->layers.size(); t.srcs = g->d_sources;
     t.step0 = (long long)step0; t.dt = dt; t.pitch = pl.pitch; t.rows = pl.rows; t.ns = pl.ns;
+    { const char* ev = getenv("AO_DBG"); t.dbg = ev ? atoi(ev) : 0; }
     return t;
 }
 
@@ -312,11 +282,11 @@ void fused_tile_shape(int M, int* G, int* R2)
 
 static size_t fused_xch_bytes(int M) { return M == 32 ? FusedCfg<32>::XCH_BYTES : FusedCfg<16>::XCH_BYTES; }
 
-bool fused_supported(const ao_geometry* g, const WfsH& w)
+bool fused_supported(const ao_geometry* g, const WfsH& w, double dt)
 {
     if (!(w.M == 16 || w.M == 32) || w.n * 2 != w.M || w.P != 8 || w.beta * w.P != w.M) return false;
     if (w.fused_items == nullptr || w.n_fused_items == 0) return false;
-    return plan_tiles(g, w.grp.src, fused_xch_bytes(w.M)).ok;
+    return plan_tiles(g, w.grp.src, dt, fused_xch_bytes(w.M)).ok;
 }
 
 template <int M>
@@ -327,17 +297,18 @@ static cudaError_t launch_fused_variant(ao_geometry* g, const WfsH& w, FusedArgs
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     const size_t nsa = (size_t)w.n_sub * w.n_sub;
-    const long long per_step = (long long)a.n_items * a.n_sel;
-    const int max_steps = (int)std::max<long long>(1, 0x7fffffffLL / per_step);
+    const long long per_pair = (long long)a.n_items * a.n_sel;
+    int max_steps = (int)std::max<long long>(2, 2 * (0x7fffffffLL / per_pair));
+    max_steps &= ~1;                                       // chunks start on an even step: pairs stay aligned
     const int64_t step0 = a.T.step0;
     for (int k0 = 0; k0 < n_steps; k0 += max_steps) {
         const int ks = n_steps - k0 < max_steps ? n_steps - k0 : max_steps;
         FusedArgs b = a;
-        b.T.step0 = step0 + k0; b.n_steps = ks;
+        b.T.step0 = step0 + k0; b.n_steps = ks; b.n_pairs = (ks + kKS - 1) / kKS;
         const size_t set0 = (size_t)k0 * a.n_sel;
         if (a.images) b.images = a.images + set0 * nsa * w.P * w.P;
         if (a.slopes) b.slopes = a.slopes + set0 * 2 * nsa;
-        kern<<<(unsigned)(per_step * ks), kFusedThreads, pl.smem, st>>>(b);
+        kern<<<(unsigned)(per_pair * b.n_pairs), kFusedThreads, pl.smem, st>>>(b);
         g->launches++;
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
@@ -347,8 +318,8 @@ static cudaError_t launch_fused_variant(ao_geometry* g, const WfsH& w, FusedArgs
 cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_steps, double dt,
                          const NoiseP& noise, float* images, float* slopes, cudaStream_t st)
 {
-    if (!fused_supported(g, w)) return cudaErrorNotSupported;
-    const TilePlan pl = plan_tiles(g, w.grp.src, fused_xch_bytes(w.M));
+    if (!fused_supported(g, w, dt)) return cudaErrorNotSupported;
+    const TilePlan pl = plan_tiles(g, w.grp.src, dt, fused_xch_bytes(w.M));
     const size_t n_sel = w.grp.src.size(), nsa = (size_t)w.n_sub * w.n_sub;
     cudaError_t e;
     // invalid subapertures are never scheduled: zero-fill the outputs first
@@ -363,37 +334,6 @@ cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_ste
     a.nz = noise; a.images = images; a.slopes = slopes;
     if (w.M == 32) return launch_fused_variant<32>(g, w, a, pl, n_steps, st);
     return launch_fused_variant<16>(g, w, a, pl, n_steps, st);
-}
-
-// Tiled ray-trace of a source group into a phase buffer; cudaErrorNotSupported if the geometry is outside
-// the fast path (the caller then uses the per-sample kernel of k_trace.cu).
-cudaError_t launch_trace_tiled(ao_geometry* g, const Group& grp, bool api_layout, long long step_stride,
-                               int64_t step0, int n_steps, double dt, float* phase, cudaStream_t st)
-{
-    const TilePlan pl = plan_tiles(g, grp.src, 0);
-    if (!pl.ok) return cudaErrorNotSupported;
-    const int n_sel = (int)grp.src.size();
-    if (n_sel == 0 || n_steps <= 0) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(k_trace_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
-    if (e != cudaSuccess) return e;
-    TiledTraceArgs a;
-    a.T = make_trace_args(g, pl, step0, dt);
-    a.sel = grp.d_src; a.off = api_layout ? grp.d_off_api : grp.d_off_stage; a.n_sel = n_sel;
-    a.step_stride = step_stride;
-    a.tiles_x = (grp.max_N + kTileCols - 1) / kTileCols;
-    a.tiles_y = (grp.max_N + kTraceRows - 1) / kTraceRows;
-    const long long per_step = (long long)a.tiles_x * a.tiles_y * n_sel;
-    const int max_steps = (int)std::max<long long>(1, 0x7fffffffLL / per_step);
-    for (int k0 = 0; k0 < n_steps; k0 += max_steps) {
-        const int ks = n_steps - k0 < max_steps ? n_steps - k0 : max_steps;
-        TiledTraceArgs b = a;
-        b.T.step0 = (long long)step0 + k0; b.n_steps = ks;
-        b.phase = phase + (size_t)k0 * step_stride;
-        k_trace_tiled<<<(unsigned)(per_step * ks), kFusedThreads, pl.smem, st>>>(b);
-        g->launches++;
-        if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    }
-    return cudaSuccess;
 }
 
 }  // namespace ao

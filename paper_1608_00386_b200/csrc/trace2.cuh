@@ -1,0 +1,310 @@
+// trace2.cuh -- tiled ray-trace core of k_fused: one CTA traces a tile of 16 output rows x 2 NT output
+// columns of one source for TWO consecutive time steps.  PAPER.md:56 (frozen flow), PAPER.md:60 (open-loop
+// wavefront of every star, finite-distance projection of the LGS); reading O2 of DESIGN.md section 3.
+//
+// Why two steps per CTA: under frozen flow the footprints of steps k and k+1 differ by a sub-pixel to
+// few-pixel wind shift, so one staged screen box (the union of both footprints) serves both; that halves the
+// L2 -> shared-memory traffic per traced sample and keeps a stage small enough for three stages in flight at
+// four CTAs per SM.
+//
+// Per layer the box is staged by TMA bulk row copies issued by warp 0 (full/empty mbarrier pipeline, no
+// CTA-wide barrier in the layer loop).  Each thread owns two columns (tid, tid + NT) packed in one 64-bit
+// register pair so that the inner loop is FFMA2 / FADD2.  Bilinear interpolation is separable: x-interpolated
+// screen rows X_r are built once per screen row, an output row costs two FFMA2.  The whole row schedule of the
+// CTA -- per (layer, step) the y-weights of the 16 rows and a bit mask "advance one screen row before row i"
+// -- is computed once in the prologue in FP64, so the branches of the row march depend on a register only.
+// Column coordinates are 32.32 fixed point: cell and fraction of column j are the two halves of
+// uf + j * du (one IMAD.WIDE), exact to 2^-32 pixel at any screen coordinate.
+// Precision: a warp-uniform piston reference (a tap of the box) is subtracted from every tap so that the fp32
+// sums stay at the few-radian level (|FFT|^2 is piston-invariant per subaperture; a warp never splits one).
+#pragma once
+#include "ao_device.cuh"
+#include "pk_tma.cuh"
+
+namespace ao {
+
+constexpr int kTR = 16;                 // output rows of a tile
+constexpr int kKS = 2;                  // time steps per CTA
+constexpr int kT2MaxStages = 4;
+
+struct Trace2Args {
+    const LayerP* layers; int n_layers;
+    const SourceP* srcs;
+    long long step0; double dt;
+    int pitch;            // staged row pitch in floats (multiple of 4)
+    int rows;             // staged rows allocated per stage (box rows + 1 prefetch pad row)
+    int ns;               // stages in flight
+    int dbg;              // experiment switch (AO_DBG): 1 = skip the row march
+};
+
+// Per active layer, built in the prologue (dynamic shared memory).
+struct __align__(16) LayerT {
+    const float* scr;     // screen base
+    int S;                // screen side
+    int cw, rw;           // start column / row of the staged box, wrapped into [0, S)
+    int wt, rt;           // box width (multiple of 4) and rows
+    unsigned duf;         // frac(du) 2^32
+    int du_hi;            // floor(du): 1 when du == 1
+    int lay;              // layer index
+    double du;            // screen pixels per output sample
+    double vrel[kKS];     // row coordinate of tile row 0 relative to box row 0
+    u64 uf[kKS];          // (column coordinate of tile column 0 - box column 0) 2^32
+    unsigned mask[kKS];   // bit i: advance one screen row before output row i
+    int roff[kKS];        // box row of the top tap of output row 0
+};
+
+struct __align__(16) Trace2Shared {
+    uint64_t full_bar[kT2MaxStages], empty_bar[kT2MaxStages];
+    int nact;
+};
+
+__host__ __device__ inline size_t trace2_sched_bytes(int n_layers)
+{
+    return (size_t)n_layers * (sizeof(LayerT) + sizeof(float4) * kKS * (kTR / 2));
+}
+
+__device__ __forceinline__ float lds_f32(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds_f32_next(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float4 lds_f32x4(uint32_t addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
+// ---- the 16 output rows of one (layer, step) as a two-state machine ----
+// The x-interpolated screen rows above and below the current output row live in the packed registers Xa
+// and Xb; in state E the top row is Xa and the bottom row Xb, in state O the roles are swapped, so that
+// advancing one screen row (new bottom row -> the register of the old top row) needs no register move.
+// The advance decision of row i is bit i of `mask` (warp-uniform, known before the march starts); the taps of
+// the next screen row are prefetched one advance ahead (p0 = left taps, p1 = right taps of the two columns).
+#define T2_ADV(XNEW)                                                                              \
+    XNEW = fma2(fx, sub2(p1, p0), sub2(p0, ref));                                                 \
+    tp0 += pb; tp1 += pb;                                                                         \
+    p0 = pack2(lds_f32(tp0), lds_f32(tp1));                                                       \
+    p1 = pack2(lds_f32_next(tp0), lds_f32_next(tp1));
+#define T2_ACC(i, W0, W1, XTOP, XBOT)                                                             \
+    acc[OFF + i] = fma2(pack2(W1, W1), XBOT, fma2(pack2(W0, W0), XTOP, acc[OFF + i]));
+#define T2_ROW(i, inext, W0, W1, PRE)                                                             \
+    LE_##i: {                                                                                     \
+        PRE                                                                                       \
+        if (mask & (1u << i)) { T2_ADV(Xa) T2_ACC(i, W0, W1, Xb, Xa) goto LO_##inext; }           \
+        T2_ACC(i, W0, W1, Xa, Xb) goto LE_##inext;                                                \
+    }                                                                                             \
+    LO_##i: {                                                                                     \
+        PRE                                                                                       \
+        if (mask & (1u << i)) { T2_ADV(Xb) T2_ACC(i, W0, W1, Xa, Xb) goto LE_##inext; }           \
+        T2_ACC(i, W0, W1, Xb, Xa) goto LO_##inext;                                                \
+    }
+#define T2_NOPRE
+#define T2_RELOAD_AB wA = lds_f32x4(wtab + 64); wB = lds_f32x4(wtab + 80);
+#define T2_RELOAD_CD wC = lds_f32x4(wtab + 96); wD = lds_f32x4(wtab + 112);
+
+// acc[OFF .. OFF+15] += the layer's contribution for one step.  tp0 / tp1: shared-memory byte addresses of the
+// left tap of the thread's two columns in the box row of the top tap of output row 0; pb: row pitch in bytes;
+// wtab: shared-memory byte address of the 16 (w0, w1) weight pairs.
+template <int OFF>
+__device__ __forceinline__ void t2_march(u64 (&acc)[kKS * kTR], const unsigned mask, uint32_t tp0, uint32_t tp1,
+                                         const uint32_t pb, const u64 fx, const u64 ref, const uint32_t wtab)
+{
+    u64 Xa, Xb, p0, p1;
+    float4 wA = lds_f32x4(wtab), wB = lds_f32x4(wtab + 16), wC = lds_f32x4(wtab + 32), wD = lds_f32x4(wtab + 48);
+    p0 = pack2(lds_f32(tp0), lds_f32(tp1));
+    p1 = pack2(lds_f32_next(tp0), lds_f32_next(tp1));
+    T2_ADV(Xa)
+    T2_ADV(Xb)
+    goto LE_0;
+    T2_ROW(0, 1, wA.x, wA.y, T2_NOPRE)   T2_ROW(1, 2, wA.z, wA.w, T2_NOPRE)
+    T2_ROW(2, 3, wB.x, wB.y, T2_NOPRE)   T2_ROW(3, 4, wB.z, wB.w, T2_NOPRE)
+    T2_ROW(4, 5, wC.x, wC.y, T2_RELOAD_AB)   T2_ROW(5, 6, wC.z, wC.w, T2_NOPRE)
+    T2_ROW(6, 7, wD.x, wD.y, T2_NOPRE)   T2_ROW(7, 8, wD.z, wD.w, T2_NOPRE)
+    T2_ROW(8, 9, wA.x, wA.y, T2_RELOAD_CD) T2_ROW(9, 10, wA.z, wA.w, T2_NOPRE)
+    T2_ROW(10, 11, wB.x, wB.y, T2_NOPRE) T2_ROW(11, 12, wB.z, wB.w, T2_NOPRE)
+    T2_ROW(12, 13, wC.x, wC.y, T2_NOPRE) T2_ROW(13, 14, wC.z, wC.w, T2_NOPRE)
+    T2_ROW(14, 15, wD.x, wD.y, T2_NOPRE) T2_ROW(15, 16, wD.z, wD.w, T2_NOPRE)
+    LE_16: LO_16: ;
+}
+
+// Ray-trace one tile for two steps: rows ifirst .. ifirst+15, columns jfirst + {tid, tid + NT} of source `sp` at
+// time steps step_first and step_first + 1.  acc[s * 16 + i] receives the packed (column tid, column tid + NT)
+// layer sums of step s, row i, minus warp-uniform piston references.
+// `dyn`: dynamic shared memory, 128-byte aligned: [ns][rows][pitch] floats, then trace2_sched_bytes(n_layers).
+// All NT threads call it.  On return every thread has finished reading the stages, but other warps may not
+// have: __syncthreads() before reusing the memory.
+template <int NT>
+__device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& sp, Trace2Shared& S, unsigned char* dyn,
+                                            const int jfirst, const int ifirst, const long long step_first,
+                                            u64 (&acc)[kKS * kTR])
+{
+    constexpr int NCOL = 2 * NT;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int pitch = A.pitch, ns = A.ns;
+    const int tile_floats = A.rows * pitch;
+    float* tiles = reinterpret_cast<float*>(dyn);
+    LayerT* L = reinterpret_cast<LayerT*>(dyn + (size_t)ns * tile_floats * sizeof(float));
+    float* W = reinterpret_cast<float*>(L + A.n_layers);          // [layer][step][row][w0, w1]
+
+    if (tid == 0) {
+        int na = 0;
+        for (int l = 0; l < A.n_layers; ++l)
+            if (A.layers[l].height < sp.H) L[na++].lay = l;
+        S.nact = na;
+        for (int s = 0; s < kT2MaxStages; ++s) { mbar_init(&S.full_bar[s], 1); mbar_init(&S.empty_bar[s], NT / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int nact = S.nact;
+
+    // ---- per-layer geometry (FP64): staged box = union of the footprints of both steps ----
+    for (int a = tid; a < nact; a += NT) {
+        LayerT& T = L[a];
+        const LayerP lp = A.layers[T.lay];
+        const double gamma = 1.0 - lp.height * sp.inv_H;
+        const double x0 = -0.5 * (double)(sp.N - 1) * sp.d;
+        const double c = 0.5 * (double)(lp.S - 1);
+        double du = gamma * sp.d * lp.inv_pitch;
+        if (fabs(du - 1.0) < 1e-9) du = 1.0;                     // same-pitch grids: exactly one pixel per sample
+        double uf[kKS], vf[kKS];
+        long long cmin = 0, cmax = 0, rmin = 0, rmax = 0;
+#pragma unroll
+        for (int s = 0; s < kKS; ++s) {
+            const double t = (double)(step_first + s) * A.dt;
+            const double u0 = (gamma * x0 + lp.height * sp.thx - lp.wx * t) * lp.inv_pitch + c;
+            const double v0 = (gamma * x0 + lp.height * sp.thy - lp.wy * t) * lp.inv_pitch + c;
+            uf[s] = fma((double)jfirst, du, u0);
+            vf[s] = fma((double)ifirst, du, v0);
+            const long long c_lo = (long long)floor(uf[s]) & ~3LL;                         // 16-byte aligned start
+            const long long c_hi = (long long)floor(fma((double)(NCOL - 1), du, uf[s])) + 2;
+            const long long r_lo = (long long)floor(vf[s]);
+            const long long r_hi = (long long)floor(fma((double)(kTR - 1), du, vf[s])) + 1;
+            if (s == 0 || c_lo < cmin) cmin = c_lo;
+            if (s == 0 || c_hi > cmax) cmax = c_hi;
+            if (s == 0 || r_lo < rmin) rmin = r_lo;
+            if (s == 0 || r_hi > rmax) rmax = r_hi;
+        }
+        int wt = (int)(cmax - cmin + 1); wt = (wt + 3) & ~3; if (wt > pitch) wt = pitch;
+        int rt = (int)(rmax - rmin + 1); if (rt > A.rows - 1) rt = A.rows - 1;
+        long long cw = cmin % lp.S; if (cw < 0) cw += lp.S;
+        long long rw = rmin % lp.S; if (rw < 0) rw += lp.S;
+        T.scr = lp.screen; T.S = lp.S; T.cw = (int)cw; T.rw = (int)rw; T.wt = wt; T.rt = rt;
+        T.du = du; T.du_hi = du >= 1.0 ? 1 : 0;
+        const unsigned long long f = __double2ull_rn((du - (double)T.du_hi) * 4294967296.0);
+        T.duf = f > 0xffffffffull ? 0xffffffffu : (unsigned)f;
+#pragma unroll
+        for (int s = 0; s < kKS; ++s) {
+            T.uf[s] = __double2ull_rn((uf[s] - (double)cmin) * 4294967296.0);
+            T.vrel[s] = vf[s] - (double)rmin;
+        }
+    }
+    __syncthreads();
+
+    // producer (warp 0): TMA bulk row copies of active layer `a` into `stage`
+    auto issue = [&](int a, int stage) {
+        const LayerT& T = L[a];
+        const int wt = T.wt, rt = T.rt, Sn = T.S, cw = T.cw, rw = T.rw;
+        const float* scr = T.scr;
+        uint64_t* bar = &S.full_bar[stage];
+        float* dst = tiles + (size_t)stage * tile_floats;
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(rt * wt) * 4u);
+        __syncwarp();
+        const int first = (cw + wt <= Sn) ? wt : Sn - cw;                     // floats before the periodic wrap
+        for (int r = lane; r < rt; r += 32) {
+            int rr = rw + r; if (rr >= Sn) rr -= Sn;
+            const float* srow = scr + (size_t)rr * Sn;
+            bulk_g2s(dst + r * pitch, srow + cw, (uint32_t)first * 4u, bar);
+            if (first < wt) bulk_g2s(dst + r * pitch + first, srow, (uint32_t)(wt - first) * 4u, bar);
+        }
+    };
+    if (warp == 0)
+        for (int a = 0; a < ns && a < nact; ++a) issue(a, a);
+
+    // ---- row schedules (FP64): y-weights, advance mask and first box row per (layer, step) ----
+    for (int t = tid; t < nact * kKS; t += NT) {
+        const int a = t / kKS, s = t - a * kKS;
+        LayerT& T = L[a];
+        const double du = T.du, vrel = T.vrel[s];
+        float* w = W + (size_t)t * (2 * kTR);
+        unsigned mask = 0;
+        long long rprev = 0;
+#pragma unroll 1
+        for (int i = 0; i < kTR; ++i) {
+            const double v = fma((double)i, du, vrel);
+            long long r = (long long)floor(v);
+            if (i == 0) T.roff[s] = (int)r;
+            else {
+                if (r > rprev + 1) r = rprev + 1;                 // rounding across a cell edge: same value by continuity
+                if (r != rprev) mask |= 1u << i;
+            }
+            rprev = r;
+            const double fy = v - (double)r;
+            w[2 * i] = (float)(1.0 - fy);
+            w[2 * i + 1] = (float)fy;
+        }
+        T.mask[s] = mask;
+    }
+
+#pragma unroll
+    for (int i = 0; i < kKS * kTR; ++i) acc[i] = 0ull;
+    __syncthreads();
+
+    const uint32_t tiles_s = smem_u32(tiles), w_s = smem_u32(W);
+    const uint32_t pb = (uint32_t)pitch * 4u, tile_bytes = (uint32_t)tile_floats * 4u;
+    const int dbg = A.dbg;
+    int stage = 0, pstage = 0;
+    uint32_t par = 0, ppar = 0;                // stage/parity of layer a and of layer a-1
+    for (int a = 0; a < nact; ++a) {
+        // refill the stage that layer a-1 used, once every warp has released it
+        if (warp == 0 && a >= 1 && a - 1 + ns < nact) {
+            mbar_wait(&S.empty_bar[pstage], ppar);
+            issue(a - 1 + ns, pstage);
+        }
+        const LayerT& T = L[a];
+        const u64 du64 = ((u64)(unsigned)T.du_hi << 32) | (u64)T.duf;
+        const u64 uf0 = T.uf[0], uf1 = T.uf[1];
+        const unsigned m0 = T.mask[0], m1 = T.mask[1];
+        const int ro0 = T.roff[0], ro1 = T.roff[1];
+        const uint32_t tile_s = tiles_s + (uint32_t)stage * tile_bytes;
+        const u64 colA = (u64)(unsigned)tid * du64, colB = colA + (u64)NT * du64;
+        const u64 colW = (u64)(unsigned)(tid & ~31) * du64;
+        mbar_wait(&S.full_bar[stage], par);
+        u64 ref;
+        {
+            const u64 a0 = uf0 + colW, a1 = a0 + (u64)NT * du64;
+            const uint32_t rowb = tile_s + (uint32_t)ro0 * pb;
+            ref = pack2(lds_f32(rowb + (uint32_t)(a0 >> 32) * 4u), lds_f32(rowb + (uint32_t)(a1 >> 32) * 4u));
+        }
+        const float k32 = 2.3283064365386963e-10f;             // 2^-32
+        if (!(dbg & 1)) {
+            {
+                const u64 U0 = uf0 + colA, U1 = uf0 + colB;
+                const u64 fx = pack2(__uint2float_rn((unsigned)U0) * k32, __uint2float_rn((unsigned)U1) * k32);
+                const uint32_t rowb = tile_s + (uint32_t)ro0 * pb;
+                t2_march<0>(acc, m0, rowb + (uint32_t)(U0 >> 32) * 4u, rowb + (uint32_t)(U1 >> 32) * 4u, pb, fx, ref,
+                            w_s + (uint32_t)(a * kKS + 0) * (2 * kTR * 4));
+            }
+            {
+                const u64 U0 = uf1 + colA, U1 = uf1 + colB;
+                const u64 fx = pack2(__uint2float_rn((unsigned)U0) * k32, __uint2float_rn((unsigned)U1) * k32);
+                const uint32_t rowb = tile_s + (uint32_t)ro1 * pb;
+                t2_march<kTR>(acc, m1, rowb + (uint32_t)(U0 >> 32) * 4u, rowb + (uint32_t)(U1 >> 32) * 4u, pb, fx, ref,
+                              w_s + (uint32_t)(a * kKS + 1) * (2 * kTR * 4));
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&S.empty_bar[stage]);
+        pstage = stage; ppar = par;
+        if (++stage == ns) { stage = 0; par ^= 1u; }
+    }
+}
+
+}  // namespace ao
