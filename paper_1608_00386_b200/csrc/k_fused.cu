@@ -222,7 +222,7 @@ struct TilePlan { bool ok; int pitch, rows, ns; size_t smem; };
 
 // Staging plan of the two-step tiled ray-trace for the sources `src` (all active layers): the union box of a
 // 16 x 256 tile over two consecutive steps must fit a shared-memory stage and the row march needs
-// 0 < du <= 1.  `min_bytes`: floor on the stage region (the exchange buffer of k_fused aliases it).
+// 1/2 <= du <= 1 (screen pixels per output sample).  `min_bytes`: floor on the stage region (the exchange buffer of k_fused aliases it).
 static TilePlan plan_tiles(const ao_geometry* g, const std::vector<int>& src, double dt, size_t min_bytes)
 {
     TilePlan pl = {false, 0, 0, 0, 0};
@@ -235,7 +235,7 @@ static TilePlan plan_tiles(const ao_geometry* g, const std::vector<int>& src, do
             if (!(lp.height < sp.H)) continue;
             double du = (1.0 - lp.height * sp.inv_H) * sp.d * lp.inv_pitch;
             if (fabs(du - 1.0) < 1e-9) du = 1.0;
-            if (!(du > 0.0) || du > 1.0) return pl;              // the row march assumes 0 < du <= 1
+            if (!(du >= 0.5) || du > 1.0) return pl;             // the row march assumes 1/2 <= du <= 1
             if (lp.S % 4 != 0) return pl;                          // 16-byte aligned rows for the bulk copies
             const double shx = fabs(lp.wx * dt * lp.inv_pitch) * (kKS - 1), shy = fabs(lp.wy * dt * lp.inv_pitch) * (kKS - 1);
             ext_x = std::max(ext_x, (kTileCols - 1) * du + shx);

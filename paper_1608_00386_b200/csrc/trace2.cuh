@@ -9,10 +9,10 @@
 //
 // Per layer the box is staged by TMA bulk row copies issued by warp 0 (full/empty mbarrier pipeline, no
 // CTA-wide barrier in the layer loop).  Each thread owns two columns (tid, tid + NT) packed in one 64-bit
-// register pair so that the inner loop is FFMA2 / FADD2.  Bilinear interpolation is separable: x-interpolated
-// screen rows X_r are built once per screen row, an output row costs two FFMA2.  The whole row schedule of the
-// CTA -- per (layer, step) the y-weights of the 16 rows and a bit mask "advance one screen row before row i"
-// -- is computed once in the prologue in FP64, so the branches of the row march depend on a register only.
+// register pair so that the inner loop is FFMA2 / FADD2.  Bilinear interpolation is separable: an output row
+// combines x-interpolated screen rows with warp-uniform y-weights.  Warp 0 writes, with each stage it issues,
+// the FP64 row table of that (layer, two steps): per output row the weights and the shared-memory offset of its
+// bottom screen row, so the row march (t2_march) is branch-free straight-line code.
 // Column coordinates are 32.32 fixed point: cell and fraction of column j are the two halves of
 // uf + j * du (one IMAD.WIDE), exact to 2^-32 pixel at any screen coordinate.
 // Precision: a warp-uniform piston reference (a tap of the box) is subtracted from every tap so that the fp32
@@ -49,8 +49,6 @@ struct __align__(16) LayerT {
     double du;            // screen pixels per output sample
     double vrel[kKS];     // row coordinate of tile row 0 relative to box row 0
     u64 uf[kKS];          // (column coordinate of tile column 0 - box column 0) 2^32
-    unsigned mask[kKS];   // bit i: advance one screen row before output row i
-    int roff[kKS];        // box row of the top tap of output row 0
 };
 
 struct __align__(16) Trace2Shared {
@@ -60,7 +58,7 @@ struct __align__(16) Trace2Shared {
 
 __host__ __device__ inline size_t trace2_sched_bytes(int n_layers)
 {
-    return (size_t)n_layers * (sizeof(LayerT) + sizeof(float4) * kKS * (kTR / 2));
+    return (size_t)n_layers * sizeof(LayerT) + (sizeof(float4) * kTR + sizeof(int) * 4) * kKS * kT2MaxStages;
 }
 
 __device__ __forceinline__ float lds_f32(uint32_t addr)
@@ -82,57 +80,39 @@ __device__ __forceinline__ float4 lds_f32x4(uint32_t addr)
     return v;
 }
 
-// ---- the 16 output rows of one (layer, step) as a two-state machine ----
-// The x-interpolated screen rows above and below the current output row live in the packed registers Xa
-// and Xb; in state E the top row is Xa and the bottom row Xb, in state O the roles are swapped, so that
-// advancing one screen row (new bottom row -> the register of the old top row) needs no register move.
-// The advance decision of row i is bit i of `mask` (warp-uniform, known before the march starts); the taps of
-// the next screen row are prefetched one advance ahead (p0 = left taps, p1 = right taps of the two columns).
-#define T2_ADV(XNEW)                                                                              \
-    XNEW = fma2(fx, sub2(p1, p0), sub2(p0, ref));                                                 \
-    tp0 += pb; tp1 += pb;                                                                         \
-    p0 = pack2(lds_f32(tp0), lds_f32(tp1));                                                       \
-    p1 = pack2(lds_f32_next(tp0), lds_f32_next(tp1));
-#define T2_ACC(i, W0, W1, XTOP, XBOT)                                                             \
-    acc[OFF + i] = fma2(pack2(W1, W1), XBOT, fma2(pack2(W0, W0), XTOP, acc[OFF + i]));
-#define T2_ROW(i, inext, W0, W1, PRE)                                                             \
-    LE_##i: {                                                                                     \
-        PRE                                                                                       \
-        if (mask & (1u << i)) { T2_ADV(Xa) T2_ACC(i, W0, W1, Xb, Xa) goto LO_##inext; }           \
-        T2_ACC(i, W0, W1, Xa, Xb) goto LE_##inext;                                                \
-    }                                                                                             \
-    LO_##i: {                                                                                     \
-        PRE                                                                                       \
-        if (mask & (1u << i)) { T2_ADV(Xb) T2_ACC(i, W0, W1, Xa, Xb) goto LE_##inext; }           \
-        T2_ACC(i, W0, W1, Xb, Xa) goto LO_##inext;                                                \
-    }
-#define T2_NOPRE
-#define T2_RELOAD_AB wA = lds_f32x4(wtab + 64); wB = lds_f32x4(wtab + 80);
-#define T2_RELOAD_CD wC = lds_f32x4(wtab + 96); wD = lds_f32x4(wtab + 112);
+// ---- the 16 output rows of one (layer, step): straight-line row march ----
+// Output row i interpolates between the x-interpolated screen rows X[r_i] (top) and X[r_i + 1] (bottom).
+// Every row builds ITS OWN bottom row N_i = X[r_i + 1] from four taps at a table-driven shared-memory offset
+// (no carried pointer, no condition).  Because 1/2 <= du <= 1, consecutive output rows advance by 0 or 1 screen
+// rows and never stall twice in a row, so the top row is N_{i-1} (advance) or N_{i-2} (no advance): the
+// prologue folds that choice into the weights, acc_i += w1 N_i + a N_{i-1} + b N_{i-2} with (a, b) =
+// (w0, 0) or (0, w0).  The march is therefore one basic block with static registers: no branch (a taken
+// branch per row starved the instruction fetch), no select, and every row's loads are independent of the
+// previous rows', so ptxas overlaps the shared-memory latency of one row with the FFMA2 chains of others.
+// Table entry of row i (16 bytes): (w1, a, b, byte offset of X[r_i + 1] relative to X[r_0]).
+__device__ __forceinline__ u64 t2_xrow(const uint32_t a0, const uint32_t a1, const u64 fx, const u64 ref)
+{
+    const u64 p0 = pack2(lds_f32(a0), lds_f32(a1));
+    const u64 p1 = pack2(lds_f32_next(a0), lds_f32_next(a1));
+    return fma2(fx, sub2(p1, p0), sub2(p0, ref));
+}
 
 // acc[OFF .. OFF+15] += the layer's contribution for one step.  tp0 / tp1: shared-memory byte addresses of the
-// left tap of the thread's two columns in the box row of the top tap of output row 0; pb: row pitch in bytes;
-// wtab: shared-memory byte address of the 16 (w0, w1) weight pairs.
+// left tap of the thread's two columns in box row r_0 (top tap of output row 0); wtab: shared-memory byte
+// address of the 16 table entries.
 template <int OFF>
-__device__ __forceinline__ void t2_march(u64 (&acc)[kKS * kTR], const unsigned mask, uint32_t tp0, uint32_t tp1,
-                                         const uint32_t pb, const u64 fx, const u64 ref, const uint32_t wtab)
+__device__ __forceinline__ void t2_march(u64 (&acc)[kKS * kTR], const uint32_t tp0, const uint32_t tp1,
+                                         const u64 fx, const u64 ref, const uint32_t wtab)
 {
-    u64 Xa, Xb, p0, p1;
-    float4 wA = lds_f32x4(wtab), wB = lds_f32x4(wtab + 16), wC = lds_f32x4(wtab + 32), wD = lds_f32x4(wtab + 48);
-    p0 = pack2(lds_f32(tp0), lds_f32(tp1));
-    p1 = pack2(lds_f32_next(tp0), lds_f32_next(tp1));
-    T2_ADV(Xa)
-    T2_ADV(Xb)
-    goto LE_0;
-    T2_ROW(0, 1, wA.x, wA.y, T2_NOPRE)   T2_ROW(1, 2, wA.z, wA.w, T2_NOPRE)
-    T2_ROW(2, 3, wB.x, wB.y, T2_NOPRE)   T2_ROW(3, 4, wB.z, wB.w, T2_NOPRE)
-    T2_ROW(4, 5, wC.x, wC.y, T2_RELOAD_AB)   T2_ROW(5, 6, wC.z, wC.w, T2_NOPRE)
-    T2_ROW(6, 7, wD.x, wD.y, T2_NOPRE)   T2_ROW(7, 8, wD.z, wD.w, T2_NOPRE)
-    T2_ROW(8, 9, wA.x, wA.y, T2_RELOAD_CD) T2_ROW(9, 10, wA.z, wA.w, T2_NOPRE)
-    T2_ROW(10, 11, wB.x, wB.y, T2_NOPRE) T2_ROW(11, 12, wB.z, wB.w, T2_NOPRE)
-    T2_ROW(12, 13, wC.x, wC.y, T2_NOPRE) T2_ROW(13, 14, wC.z, wC.w, T2_NOPRE)
-    T2_ROW(14, 15, wD.x, wD.y, T2_NOPRE) T2_ROW(15, 16, wD.z, wD.w, T2_NOPRE)
-    LE_16: LO_16: ;
+    u64 n1 = t2_xrow(tp0, tp1, fx, ref), n2 = n1;
+#pragma unroll
+    for (int i = 0; i < kTR; ++i) {
+        const float4 w = lds_f32x4(wtab + 16u * (uint32_t)i);
+        const uint32_t off = __float_as_uint(w.w);
+        const u64 n0 = t2_xrow(tp0 + off, tp1 + off, fx, ref);
+        acc[OFF + i] = fma2(pack2(w.x, w.x), n0, fma2(pack2(w.y, w.y), n1, fma2(pack2(w.z, w.z), n2, acc[OFF + i])));
+        n2 = n1; n1 = n0;
+    }
 }
 
 // Ray-trace one tile for two steps: rows ifirst .. ifirst+15, columns jfirst + {tid, tid + NT} of source `sp` at
@@ -152,7 +132,8 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
     const int tile_floats = A.rows * pitch;
     float* tiles = reinterpret_cast<float*>(dyn);
     LayerT* L = reinterpret_cast<LayerT*>(dyn + (size_t)ns * tile_floats * sizeof(float));
-    float* W = reinterpret_cast<float*>(L + A.n_layers);          // [layer][step][row][w0, w1]
+    float4* Wt = reinterpret_cast<float4*>(L + A.n_layers);       // [stage][step][row] table entries
+    int* R0 = reinterpret_cast<int*>(Wt + kT2MaxStages * kKS * kTR);   // [stage][step] box row of the top tap of row 0
 
     if (tid == 0) {
         int na = 0;
@@ -215,6 +196,25 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         const float* scr = T.scr;
         uint64_t* bar = &S.full_bar[stage];
         float* dst = tiles + (size_t)stage * tile_floats;
+        {   // row table of this stage: lane = step * 16 + row (FP64)
+            static_assert(kKS * kTR == 32, "one lane per (step, row)");
+            const int s = lane / kTR, i = lane - s * kTR;
+            const double v = fma((double)i, T.du, T.vrel[s]);
+            long long r = (long long)floor(v);
+            const long long rprev = __shfl_up_sync(0xffffffffu, r, 1);
+            const long long r0 = __shfl_sync(0xffffffffu, r, s * kTR);
+            bool adv = true;
+            if (i > 0) {
+                if (r > rprev + 1) r = rprev + 1;                 // rounding across a cell edge: same value by continuity
+                adv = r != rprev;
+            }
+            const double fy = v - (double)r;
+            const float w0 = (float)(1.0 - fy);
+            Wt[stage * (kKS * kTR) + lane] = make_float4((float)fy, adv ? w0 : 0.0f, adv ? 0.0f : w0,
+                                                          __uint_as_float((uint32_t)((int)(r + 1 - r0) * pitch * 4)));
+            if (i == 0) R0[stage * kKS + s] = (int)r;
+        }
+        __syncwarp();
         if (lane == 0) mbar_expect_tx(bar, (uint32_t)(rt * wt) * 4u);
         __syncwarp();
         const int first = (cw + wt <= Sn) ? wt : Sn - cw;                     // floats before the periodic wrap
@@ -228,36 +228,11 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
     if (warp == 0)
         for (int a = 0; a < ns && a < nact; ++a) issue(a, a);
 
-    // ---- row schedules (FP64): y-weights, advance mask and first box row per (layer, step) ----
-    for (int t = tid; t < nact * kKS; t += NT) {
-        const int a = t / kKS, s = t - a * kKS;
-        LayerT& T = L[a];
-        const double du = T.du, vrel = T.vrel[s];
-        float* w = W + (size_t)t * (2 * kTR);
-        unsigned mask = 0;
-        long long rprev = 0;
-#pragma unroll 1
-        for (int i = 0; i < kTR; ++i) {
-            const double v = fma((double)i, du, vrel);
-            long long r = (long long)floor(v);
-            if (i == 0) T.roff[s] = (int)r;
-            else {
-                if (r > rprev + 1) r = rprev + 1;                 // rounding across a cell edge: same value by continuity
-                if (r != rprev) mask |= 1u << i;
-            }
-            rprev = r;
-            const double fy = v - (double)r;
-            w[2 * i] = (float)(1.0 - fy);
-            w[2 * i + 1] = (float)fy;
-        }
-        T.mask[s] = mask;
-    }
-
 #pragma unroll
     for (int i = 0; i < kKS * kTR; ++i) acc[i] = 0ull;
     __syncthreads();
 
-    const uint32_t tiles_s = smem_u32(tiles), w_s = smem_u32(W);
+    const uint32_t tiles_s = smem_u32(tiles), w_s = smem_u32(Wt);
     const uint32_t pb = (uint32_t)pitch * 4u, tile_bytes = (uint32_t)tile_floats * 4u;
     const int dbg = A.dbg;
     int stage = 0, pstage = 0;
@@ -271,12 +246,11 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         const LayerT& T = L[a];
         const u64 du64 = ((u64)(unsigned)T.du_hi << 32) | (u64)T.duf;
         const u64 uf0 = T.uf[0], uf1 = T.uf[1];
-        const unsigned m0 = T.mask[0], m1 = T.mask[1];
-        const int ro0 = T.roff[0], ro1 = T.roff[1];
         const uint32_t tile_s = tiles_s + (uint32_t)stage * tile_bytes;
         const u64 colA = (u64)(unsigned)tid * du64, colB = colA + (u64)NT * du64;
         const u64 colW = (u64)(unsigned)(tid & ~31) * du64;
         mbar_wait(&S.full_bar[stage], par);
+        const int ro0 = R0[stage * kKS], ro1 = R0[stage * kKS + 1];
         u64 ref;
         {
             const u64 a0 = uf0 + colW, a1 = a0 + (u64)NT * du64;
@@ -289,15 +263,15 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
                 const u64 U0 = uf0 + colA, U1 = uf0 + colB;
                 const u64 fx = pack2(__uint2float_rn((unsigned)U0) * k32, __uint2float_rn((unsigned)U1) * k32);
                 const uint32_t rowb = tile_s + (uint32_t)ro0 * pb;
-                t2_march<0>(acc, m0, rowb + (uint32_t)(U0 >> 32) * 4u, rowb + (uint32_t)(U1 >> 32) * 4u, pb, fx, ref,
-                            w_s + (uint32_t)(a * kKS + 0) * (2 * kTR * 4));
+                t2_march<0>(acc, rowb + (uint32_t)(U0 >> 32) * 4u, rowb + (uint32_t)(U1 >> 32) * 4u, fx, ref,
+                            w_s + (uint32_t)(stage * kKS + 0) * (kTR * 16));
             }
             {
                 const u64 U0 = uf1 + colA, U1 = uf1 + colB;
                 const u64 fx = pack2(__uint2float_rn((unsigned)U0) * k32, __uint2float_rn((unsigned)U1) * k32);
                 const uint32_t rowb = tile_s + (uint32_t)ro1 * pb;
-                t2_march<kTR>(acc, m1, rowb + (uint32_t)(U0 >> 32) * 4u, rowb + (uint32_t)(U1 >> 32) * 4u, pb, fx, ref,
-                              w_s + (uint32_t)(a * kKS + 1) * (2 * kTR * 4));
+                t2_march<kTR>(acc, rowb + (uint32_t)(U0 >> 32) * 4u, rowb + (uint32_t)(U1 >> 32) * 4u, fx, ref,
+                              w_s + (uint32_t)(stage * kKS + 1) * (kTR * 16));
             }
         }
         __syncwarp();
