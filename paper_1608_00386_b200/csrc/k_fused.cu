@@ -27,6 +27,7 @@
 
 #include "fft_reg.cuh"
 #include "trace2.cuh"
+#include "trace2_plan.cuh"
 
 namespace ao {
 
@@ -64,8 +65,6 @@ struct FusedArgs {
     float* slopes;                    // nullable [k][si][2][nsa]
 };
 
-constexpr int kFusedThreads = 128;
-constexpr int kTileCols = 2 * kFusedThreads;
 
 template <int M>
 struct FusedCfg {
@@ -104,7 +103,8 @@ k_fused(const FusedArgs A)
 
     // ---- phase A: ray-trace of the 16 x 256 tile, two steps, into registers ----
     u64 acc[kKS * kTR];
-    trace2_tile<NT>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc);
+    double refsum[2];                                      // unused: |FFT|^2 is piston-invariant per subaperture
+    trace2_tile<NT, false>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, refsum);
     __syncthreads();                                       // stages are dead: shared memory becomes the exchange buffer
 
     // ---- phase B: image formation, one (subaperture row, column slot) round at a time ----
@@ -113,7 +113,7 @@ k_fused(const FusedArgs A)
     const int g = tid / n, b = tid - g * n;                // subaperture in round, column in subaperture
     float2* xs = xch + (size_t)g * K::SUB_STRIDE;
 #pragma unroll 1
-    for (int rd = 0; rd < K::ROUNDS; ++rd) {
+    for (int rd = (A.T.dbg & 4) ? K::ROUNDS : 0; rd < K::ROUNDS; ++rd) {
         const int hs = rd >> 1, c = rd & 1;                // hs = step-in-pair * R2 + subaperture row
         const int sp2 = hs / R2, h = hs - sp2 * R2;
         const int k = 2 * kp + sp2;
@@ -218,60 +218,6 @@ k_fused(const FusedArgs A)
 
 // ------------------------------------------------------------------------------------------------
 // host side
-struct TilePlan { bool ok; int pitch, rows, ns; size_t smem; };
-
-// Staging plan of the two-step tiled ray-trace for the sources `src` (all active layers): the union box of a
-// 16 x 256 tile over two consecutive steps must fit a shared-memory stage and the row march needs
-// 1/2 <= du <= 1 (screen pixels per output sample).  `min_bytes`: floor on the stage region (the exchange buffer of k_fused aliases it).
-static TilePlan plan_tiles(const ao_geometry* g, const std::vector<int>& src, double dt, size_t min_bytes)
-{
-    TilePlan pl = {false, 0, 0, 0, 0};
-    double ext_x = 0.0, ext_y = 0.0;                               // box extent beyond the taps, screen pixels
-    int s_min = 1 << 30;
-    bool any = false;
-    for (int s : src) {
-        const SourceP& sp = g->sources[s];
-        for (const LayerP& lp : g->layers) {
-            if (!(lp.height < sp.H)) continue;
-            double du = (1.0 - lp.height * sp.inv_H) * sp.d * lp.inv_pitch;
-            if (fabs(du - 1.0) < 1e-9) du = 1.0;
-            if (!(du >= 0.5) || du > 1.0) return pl;             // the row march assumes 1/2 <= du <= 1
-            if (lp.S % 4 != 0) return pl;                          // 16-byte aligned rows for the bulk copies
-            const double shx = fabs(lp.wx * dt * lp.inv_pitch) * (kKS - 1), shy = fabs(lp.wy * dt * lp.inv_pitch) * (kKS - 1);
-            ext_x = std::max(ext_x, (kTileCols - 1) * du + shx);
-            ext_y = std::max(ext_y, (kTR - 1) * du + shy);
-            if (lp.S < s_min) s_min = lp.S;
-            any = true;
-        }
-    }
-    if (!any) { ext_x = kTileCols - 1; ext_y = kTR - 1; }
-    if (!(ext_x < 4096.0 && ext_y < 4096.0)) return pl;            // absurd wind shift per step: not this path
-    pl.pitch = (((int)ceil(ext_x) + 8) + 3) & ~3;                  // + alignment (3), right tap, rounding slack
-    pl.rows = (int)ceil(ext_y) + 3 + 1;                            // box rows + one prefetch pad row
-    if (s_min < pl.pitch || s_min < pl.rows) return pl;            // a box row may wrap the screen edge once only
-    const size_t stage = (size_t)pl.rows * pl.pitch * sizeof(float);
-    const size_t sched = trace2_sched_bytes((int)g->layers.size());
-    // 4 CTAs per SM: <= ~55 KB of shared memory each; as many stages (<= 4) as fit, at least 2
-    const size_t budget = 55 * 1024 + 512;
-    pl.ns = 2;
-    while (pl.ns < kT2MaxStages && (pl.ns + 1) * stage + sched + 128 + 256 <= budget) ++pl.ns;
-    if (const char* ev = getenv("AO_FUSED_STAGES")) { const int v = atoi(ev); if (v >= 2 && v <= kT2MaxStages) pl.ns = v; }
-    size_t region = pl.ns * stage;
-    if (region < min_bytes) region = (min_bytes + 15) & ~(size_t)15;
-    pl.smem = region + sched + 128;
-    pl.ok = pl.smem <= 200 * 1024;
-    return pl;
-}
-
-static Trace2Args make_trace_args(const ao_geometry* g, const TilePlan& pl, int64_t step0, double dt)
-{
-    Trace2Args t;
-    t.layers = g->d_layers; t.n_layers = (int)g->layers.size(); t.srcs = g->d_sources;
-    t.step0 = (long long)step0; t.dt = dt; t.pitch = pl.pitch; t.rows = pl.rows; t.ns = pl.ns;
-    { const char* ev = getenv("AO_DBG"); t.dbg = ev ? atoi(ev) : 0; }
-    return t;
-}
-
 // Tile shape of the fused kernel per FFT size: G subapertures wide, R2 subaperture rows tall.
 void fused_tile_shape(int M, int* G, int* R2)
 {
@@ -286,11 +232,11 @@ bool fused_supported(const ao_geometry* g, const WfsH& w, double dt)
 {
     if (!(w.M == 16 || w.M == 32) || w.n * 2 != w.M || w.P != 8 || w.beta * w.P != w.M) return false;
     if (w.fused_items == nullptr || w.n_fused_items == 0) return false;
-    return plan_tiles(g, w.grp.src, dt, fused_xch_bytes(w.M)).ok;
+    return plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M)).ok;
 }
 
 template <int M>
-static cudaError_t launch_fused_variant(ao_geometry* g, const WfsH& w, FusedArgs a, const TilePlan& pl, int n_steps,
+static cudaError_t launch_fused_variant(ao_geometry* g, const WfsH& w, FusedArgs a, const Tile2Plan& pl, int n_steps,
                                         cudaStream_t st)
 {
     auto kern = a.nz.on ? k_fused<M, true> : k_fused<M, false>;
@@ -319,14 +265,14 @@ cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_ste
                          const NoiseP& noise, float* images, float* slopes, cudaStream_t st)
 {
     if (!fused_supported(g, w, dt)) return cudaErrorNotSupported;
-    const TilePlan pl = plan_tiles(g, w.grp.src, dt, fused_xch_bytes(w.M));
+    const Tile2Plan pl = plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M));
     const size_t n_sel = w.grp.src.size(), nsa = (size_t)w.n_sub * w.n_sub;
     cudaError_t e;
     // invalid subapertures are never scheduled: zero-fill the outputs first
     if (images && (e = cudaMemsetAsync(images, 0, sizeof(float) * n_steps * n_sel * nsa * w.P * w.P, st)) != cudaSuccess) return e;
     if (slopes && (e = cudaMemsetAsync(slopes, 0, sizeof(float) * n_steps * n_sel * 2 * nsa, st)) != cudaSuccess) return e;
     FusedArgs a;
-    a.T = make_trace_args(g, pl, step0, dt);
+    a.T = make_trace2_args(g, pl, step0, dt);
     a.sel = w.grp.d_src; a.n_sel = (int)n_sel;
     a.items = (const WorkItem*)w.fused_items; a.n_items = w.n_fused_items; a.n_steps = n_steps;
     a.amp = w.d_amp; a.valid = w.d_valid; a.n_sub = w.n_sub;

@@ -7,11 +7,9 @@
 #include <vector>
 
 #include "trace_tile.cuh"
+#include "trace2_plan.cuh"
 
 namespace ao {
-
-constexpr int kFusedThreads = 128;
-constexpr int kTileCols = 2 * kFusedThreads;
 
 // ------------------------------------------------------------------------------------------------
 // k_trace_tiled: the same tiled ray-trace, phase written to HBM (absolute: the FP64 piston sum is added back).
@@ -49,6 +47,53 @@ k_trace_tiled(const TiledTraceArgs A)
             const float2 f = unpack2(acc[i]);
             if (j0 < sp.N) out[(size_t)row * sp.N + j0] = (float)(((double)f.x + refsum[0]) * sp.scale);
             if (j1 < sp.N) out[(size_t)row * sp.N + j1] = (float)(((double)f.y + refsum[1]) * sp.scale);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// k_trace_tiled2: two-step tiles of trace2.cuh (1/2 <= du <= 1: the NGS sensors and science directions, whose
+// grids have the screen pitch, and the LGS sensors), phase written to HBM.  Absolute phase: the FP64 sum of the
+// per-layer piston references is added back.
+struct TiledTrace2Args {
+    Trace2Args T;
+    const int* sel; const long long* off; int n_sel;
+    long long step_stride;
+    int n_steps, n_pairs, tiles_x, tiles_y;
+    float* phase;
+};
+
+__global__ void __launch_bounds__(kFusedThreads, 4)
+k_trace_tiled2(const TiledTrace2Args A)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ Trace2Shared S;
+    const int tid = threadIdx.x;
+    const int kp = (int)(blockIdx.x % (unsigned)A.n_pairs);
+    unsigned rest = blockIdx.x / (unsigned)A.n_pairs;
+    const int tx = (int)(rest % (unsigned)A.tiles_x); rest /= (unsigned)A.tiles_x;
+    const int ty = (int)(rest % (unsigned)A.tiles_y);
+    const int si = (int)(rest / (unsigned)A.tiles_y);
+    const SourceP sp = A.T.srcs[A.sel[si]];
+    const int jfirst = tx * kTileCols, ifirst = ty * kTR;
+    if (jfirst >= sp.N || ifirst >= sp.N) return;          // CTA-uniform
+    u64 acc[kKS * kTR];
+    double refsum[2];
+    trace2_tile<kFusedThreads, true>(A.T, sp, S, smem, jfirst, ifirst, A.T.step0 + 2 * kp, acc, refsum);
+    const int j0 = jfirst + tid, j1 = j0 + kFusedThreads;
+#pragma unroll
+    for (int s = 0; s < kKS; ++s) {
+        const int k = 2 * kp + s;
+        if (k >= A.n_steps) break;
+        float* out = A.phase + (size_t)k * A.step_stride + A.off[si];
+#pragma unroll
+        for (int i = 0; i < kTR; ++i) {
+            const int row = ifirst + i;
+            if (row < sp.N) {
+                const float2 f = unpack2(acc[s * kTR + i]);
+                if (j0 < sp.N) out[(size_t)row * sp.N + j0] = (float)(((double)f.x + refsum[0]) * sp.scale);
+                if (j1 < sp.N) out[(size_t)row * sp.N + j1] = (float)(((double)f.y + refsum[1]) * sp.scale);
+            }
         }
     }
 }
@@ -105,10 +150,34 @@ static TraceArgs make_trace_args(const ao_geometry* g, const TilePlan& pl, int64
 cudaError_t launch_trace_tiled(ao_geometry* g, const Group& grp, bool api_layout, long long step_stride,
                                int64_t step0, int n_steps, double dt, float* phase, cudaStream_t st)
 {
-    const TilePlan pl = plan_tiles(g, grp.src, 0);
-    if (!pl.ok) return cudaErrorNotSupported;
     const int n_sel = (int)grp.src.size();
     if (n_sel == 0 || n_steps <= 0) return cudaSuccess;
+    const Tile2Plan p2 = plan_tiles2(g, grp.src, dt, 0);
+    if (p2.ok && !getenv("AO_TRACE_OLD")) {
+        cudaError_t e2 = cudaFuncSetAttribute(k_trace_tiled2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p2.smem);
+        if (e2 != cudaSuccess) return e2;
+        TiledTrace2Args a;
+        a.T = make_trace2_args(g, p2, step0, dt);
+        a.sel = grp.d_src; a.off = api_layout ? grp.d_off_api : grp.d_off_stage; a.n_sel = n_sel;
+        a.step_stride = step_stride;
+        a.tiles_x = (grp.max_N + kTileCols - 1) / kTileCols;
+        a.tiles_y = (grp.max_N + kTR - 1) / kTR;
+        const long long per_pair = (long long)a.tiles_x * a.tiles_y * n_sel;
+        int max_steps = (int)std::max<long long>(2, 2 * (0x7fffffffLL / per_pair));
+        max_steps &= ~1;
+        for (int k0 = 0; k0 < n_steps; k0 += max_steps) {
+            const int ks = n_steps - k0 < max_steps ? n_steps - k0 : max_steps;
+            TiledTrace2Args b = a;
+            b.T.step0 = (long long)step0 + k0; b.n_steps = ks; b.n_pairs = (ks + kKS - 1) / kKS;
+            b.phase = phase + (size_t)k0 * step_stride;
+            k_trace_tiled2<<<(unsigned)(per_pair * b.n_pairs), kFusedThreads, p2.smem, st>>>(b);
+            g->launches++;
+            if ((e2 = cudaGetLastError()) != cudaSuccess) return e2;
+        }
+        return cudaSuccess;
+    }
+    const TilePlan pl = plan_tiles(g, grp.src, 0);
+    if (!pl.ok) return cudaErrorNotSupported;
     cudaError_t e = cudaFuncSetAttribute(k_trace_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     TiledTraceArgs a;

@@ -34,7 +34,7 @@ struct Trace2Args {
     int pitch;            // staged row pitch in floats (multiple of 4)
     int rows;             // staged rows allocated per stage (box rows + 1 prefetch pad row)
     int ns;               // stages in flight
-    int dbg;              // experiment switch (AO_DBG): 1 = skip the row march
+    int dbg;              // experiment switch (AO_DBG): 1 = skip the row march, 2 = skip staging, 4 = skip image formation
 };
 
 // Per active layer, built in the prologue (dynamic shared memory).
@@ -59,25 +59,6 @@ struct __align__(16) Trace2Shared {
 __host__ __device__ inline size_t trace2_sched_bytes(int n_layers)
 {
     return (size_t)n_layers * sizeof(LayerT) + (sizeof(float4) * kTR + sizeof(int) * 4) * kKS * kT2MaxStages;
-}
-
-__device__ __forceinline__ float lds_f32(uint32_t addr)
-{
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ float lds_f32_next(uint32_t addr)
-{
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ float4 lds_f32x4(uint32_t addr)
-{
-    float4 v;
-    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
-    return v;
 }
 
 // ---- the 16 output rows of one (layer, step): straight-line row march ----
@@ -117,14 +98,15 @@ __device__ __forceinline__ void t2_march(u64 (&acc)[kKS * kTR], const uint32_t t
 
 // Ray-trace one tile for two steps: rows ifirst .. ifirst+15, columns jfirst + {tid, tid + NT} of source `sp` at
 // time steps step_first and step_first + 1.  acc[s * 16 + i] receives the packed (column tid, column tid + NT)
-// layer sums of step s, row i, minus warp-uniform piston references.
+// layer sums of step s, row i, minus warp-uniform piston references (the same for both steps); with REFSUM
+// their FP64 sums over the layers are returned in refsum[column] so that callers can restore absolute phase.
 // `dyn`: dynamic shared memory, 128-byte aligned: [ns][rows][pitch] floats, then trace2_sched_bytes(n_layers).
 // All NT threads call it.  On return every thread has finished reading the stages, but other warps may not
 // have: __syncthreads() before reusing the memory.
-template <int NT>
+template <int NT, bool REFSUM>
 __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& sp, Trace2Shared& S, unsigned char* dyn,
                                             const int jfirst, const int ifirst, const long long step_first,
-                                            u64 (&acc)[kKS * kTR])
+                                            u64 (&acc)[kKS * kTR], double (&refsum)[2])
 {
     constexpr int NCOL = 2 * NT;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -189,7 +171,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
     }
     __syncthreads();
 
-    // producer (warp 0): TMA bulk row copies of active layer `a` into `stage`
+    // producer (one warp): row table + TMA bulk row copies of active layer `a` into `stage`
     auto issue = [&](int a, int stage) {
         const LayerT& T = L[a];
         const int wt = T.wt, rt = T.rt, Sn = T.S, cw = T.cw, rw = T.rw;
@@ -215,6 +197,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             if (i == 0) R0[stage * kKS + s] = (int)r;
         }
         __syncwarp();
+        if (A.dbg & 2) return;
         if (lane == 0) mbar_expect_tx(bar, (uint32_t)(rt * wt) * 4u);
         __syncwarp();
         const int first = (cw + wt <= Sn) ? wt : Sn - cw;                     // floats before the periodic wrap
@@ -230,6 +213,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
 
 #pragma unroll
     for (int i = 0; i < kKS * kTR; ++i) acc[i] = 0ull;
+    refsum[0] = 0.0; refsum[1] = 0.0;
     __syncthreads();
 
     const uint32_t tiles_s = smem_u32(tiles), w_s = smem_u32(Wt);
@@ -238,8 +222,9 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
     int stage = 0, pstage = 0;
     uint32_t par = 0, ppar = 0;                // stage/parity of layer a and of layer a-1
     for (int a = 0; a < nact; ++a) {
-        // refill the stage that layer a-1 used, once every warp has released it
-        if (warp == 0 && a >= 1 && a - 1 + ns < nact) {
+        // refill the stage that layer a-1 used, once every warp has released it.  The producer role rotates:
+        // a fixed producer warp lags by its issue + table time every layer and paces the whole CTA.
+        if (warp == (a & (NT / 32 - 1)) && a >= 1 && a - 1 + ns < nact) {     // producer role rotates over the warps
             mbar_wait(&S.empty_bar[pstage], ppar);
             issue(a - 1 + ns, pstage);
         }
@@ -249,13 +234,15 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         const uint32_t tile_s = tiles_s + (uint32_t)stage * tile_bytes;
         const u64 colA = (u64)(unsigned)tid * du64, colB = colA + (u64)NT * du64;
         const u64 colW = (u64)(unsigned)(tid & ~31) * du64;
-        mbar_wait(&S.full_bar[stage], par);
+        if (!(A.dbg & 2)) mbar_wait(&S.full_bar[stage], par);
         const int ro0 = R0[stage * kKS], ro1 = R0[stage * kKS + 1];
         u64 ref;
         {
             const u64 a0 = uf0 + colW, a1 = a0 + (u64)NT * du64;
             const uint32_t rowb = tile_s + (uint32_t)ro0 * pb;
-            ref = pack2(lds_f32(rowb + (uint32_t)(a0 >> 32) * 4u), lds_f32(rowb + (uint32_t)(a1 >> 32) * 4u));
+            const float r0f = lds_f32(rowb + (uint32_t)(a0 >> 32) * 4u), r1f = lds_f32(rowb + (uint32_t)(a1 >> 32) * 4u);
+            ref = pack2(r0f, r1f);
+            if (REFSUM) { refsum[0] += (double)r0f; refsum[1] += (double)r1f; }
         }
         const float k32 = 2.3283064365386963e-10f;             // 2^-32
         if (!(dbg & 1)) {

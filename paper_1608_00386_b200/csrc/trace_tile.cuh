@@ -47,19 +47,6 @@ struct __align__(16) TraceShared {
     int nact;
 };
 
-__device__ __forceinline__ float lds_f32(uint32_t addr)
-{
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ float lds_f32_next(uint32_t addr)
-{
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v) : "r"(addr));
-    return v;
-}
-
 // The 32 output rows of a layer as a two-state machine.  The x-interpolated screen rows above and below
 // the current output row live in the packed registers Xa and Xb; in state E the top row is Xa and the
 // bottom row Xb, in state O the roles are swapped, so that advancing one screen row (new bottom row ->
