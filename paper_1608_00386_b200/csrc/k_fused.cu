@@ -36,17 +36,53 @@ namespace ao {
 // First DIF stage on the half-zero input: X[2k'] = FFT_n(e[a] cis(pi (M-1) a/M))[k'],
 //                                         X[2k'+1] = FFT_n(e[a] cis(pi (M-3) a/M))[k'].
 // `sink(k, value)` is called once for every k (k as std::integral_constant).
+// Packed-complex variant of fft_stage (fft_reg.cuh): a complex number is one f32x2 register pair, so the
+// butterfly add and subtract are one FADD2 each; twiddle multiplications stay scalar.
+template <int NUM, int DEN>
+__device__ __forceinline__ u64 cmul_cis_pk(const u64 x)
+{
+    using W = Cis<NUM, DEN>;
+    if constexpr (W::q == 0) return x;
+    else { const float2 r = cmul_cis<NUM, DEN>(unpack2(x)); return pack2(r.x, r.y); }
+}
+template <int N, int HALF>
+__device__ __forceinline__ void fft_stage_pk(u64 (&x)[N])
+{
+    static_for<0, N / 2>([&](auto bi) {
+        constexpr int b = decltype(bi)::value;
+        constexpr int grp = b / HALF, pos = b % HALF, i = grp * 2 * HALF + pos, j = i + HALF;
+        const u64 a = x[i], c = x[j];
+        x[i] = add2(a, c);
+        x[j] = cmul_cis_pk<-pos, HALF>(sub2(a, c));                            // * exp(-2 pi i pos/(2 HALF))
+    });
+    if constexpr (HALF > 1) fft_stage_pk<N, HALF / 2>(x);
+}
+
 template <int M, typename Sink>
 __device__ __forceinline__ void dft_half_padded(const float2 (&e)[M / 2], Sink&& sink)
 {
     constexpr int n = M / 2;
-    float2 y[n];
-    static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; y[a] = cmul_cis<(M - 1) * a, M>(e[a]); });
-    fft_stage<n, n / 2>(y);
-    static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k>{}, y[bitrev_c(k, n)]); });
-    static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; y[a] = cmul_cis<(M - 3) * a, M>(e[a]); });
-    fft_stage<n, n / 2>(y);
-    static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k + 1>{}, y[bitrev_c(k, n)]); });
+    u64 y[n];
+    static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; const float2 t = cmul_cis<(M - 1) * a, M>(e[a]); y[a] = pack2(t.x, t.y); });
+    fft_stage_pk<n, n / 2>(y);
+    static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k>{}, unpack2(y[bitrev_c(k, n)])); });
+    static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; const float2 t = cmul_cis<(M - 3) * a, M>(e[a]); y[a] = pack2(t.x, t.y); });
+    fft_stage_pk<n, n / 2>(y);
+    static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k + 1>{}, unpack2(y[bitrev_c(k, n)])); });
+}
+
+// sin and cos of a phase of up to a few hundred radians: exact two-constant reduction to r = x/(2 pi) - k in
+// [-1/2, 1/2] revolutions, then the SFU (sin.approx / cos.approx on [-pi, pi]: absolute error ~4e-7, which the
+// images see as a relative error of the same size; DESIGN.md section 5 "precision budget").
+__device__ __forceinline__ void sincos_reduced(const float x, float* s, float* c)
+{
+    const float kInv2PiHi = 0.15915493667125702f, kInv2PiLo = 6.4206383266e-09f;
+    const float k = rintf(x * kInv2PiHi);
+    float r = fmaf(x, kInv2PiHi, -k);
+    r = fmaf(x, kInv2PiLo, r);
+    const float a = r * 6.283185307179586f;
+    *s = __sinf(a);
+    *c = __cosf(a);
 }
 
 struct WorkItem { int p, q0, cnt, pad; };
@@ -137,7 +173,7 @@ k_fused(const FusedArgs A)
                 const float ph = (c ? f.y : f.x) * scale;
                 const float Am = active ? __ldg(ap + (size_t)i * N) : 0.0f;
                 float s, co;
-                sincosf(ph, &s, &co);
+                sincos_reduced(ph, &s, &co);
                 e[i] = make_float2(Am * co, Am * s);
             }
             dft_half_padded<M>(e, [&](auto ki, const float2 v) {
