@@ -135,7 +135,7 @@ k_big_rows(const BigRowArgs A)
             if (row_on && i < n) {
                 const float Am = __ldg(am + i);
                 float s, c;
-                sincosf(__ldg(ph + i), &s, &c);
+                sincos_reduced(__ldg(ph + i), &s, &c);
                 const float2 w = cmulf(pa, __ldg(A.pre + i));
                 v = cmulf(make_float2(Am * c, Am * s), w);
             }
@@ -192,26 +192,38 @@ k_big_cols(const BigColArgs A)
             }
         }
     } else {
-        __shared__ float pix[1024];
         const int sa = (int)(b % A.nsa);
         if (A.valid && !A.valid[sa]) {
             for (int r = tid; r < A.P; r += blockDim.x) A.out[((size_t)b * A.P + r) * A.P + g] = 0.0f;
             return;
         }
-        for (int r = tid; r < A.P; r += blockDim.x) pix[r] = 0.0f;
-        __syncthreads();
         const int m0 = A.k0 + g * A.beta;
         const float2* Tb = A.T + (size_t)b * n * M + m0 + c;
-        const int kend = A.k0 + A.beta * A.P;
+        float I[16];
         big_fft<LOGM>(tb, sm, C, c, A.tw,
             [&](int i) { return i < n ? __ldg(Tb + (size_t)i * M) : make_float2(0.0f, 0.0f); },
-            [&](int i, const float2 x, int) {
-                float I = fmaf(x.x, x.x, x.y * x.y);
-                for (int o = 1; o < C; o <<= 1) I += __shfl_xor_sync(0xffffffffu, I, o);   // the beta columns
-                if (c == 0 && i >= A.k0 && i < kend) atomicAdd(&pix[(i - A.k0) / A.beta], I);
-            });
+            [&](int, const float2 x, int slot) { I[slot] = fmaf(x.x, x.x, x.y * x.y); });
+        __syncthreads();                                      // every thread has finished reading the exchange buffer
+        // intensities to shared memory as Ib[i][c] (replaying the index arithmetic of the last pass), then one
+        // warp per detector pixel sums its beta x beta block, which is beta * C contiguous floats
+        float* Ib = reinterpret_cast<float*>(sm);
+        constexpr int RL = K::R2 == 1 ? K::R1 : K::R2, NSL = K::R2 == 1 ? 16 : 256, Q = 16 / RL;
+#pragma unroll
+        for (int q = 0; q < Q; ++q) {
+            const int bb = tb + q * K::T;
+            const int o0 = (bb / NSL) * (NSL * RL) + (bb & (NSL - 1));
+#pragma unroll
+            for (int kk = 0; kk < RL; ++kk) Ib[(o0 + kk * NSL) * C + c] = I[q * RL + kk];
+        }
         __syncthreads();
-        for (int r = tid; r < A.P; r += blockDim.x) A.out[((size_t)b * A.P + r) * A.P + g] = pix[r] * A.norm;
+        const int lane = tid & 31, warp = tid >> 5, nw = (int)(blockDim.x >> 5), span = A.beta * C;
+        for (int r = warp; r < A.P; r += nw) {
+            const float* src = Ib + (size_t)(A.k0 + r * A.beta) * C;
+            float s = 0.0f;
+            for (int e = lane; e < span; e += 32) s += src[e];
+            s = warp_sum(s);
+            if (lane == 0) A.out[((size_t)b * A.P + r) * A.P + g] = s * A.norm;
+        }
     }
 }
 

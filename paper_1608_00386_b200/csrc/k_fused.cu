@@ -71,20 +71,6 @@ __device__ __forceinline__ void dft_half_padded(const float2 (&e)[M / 2], Sink&&
     static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k + 1>{}, unpack2(y[bitrev_c(k, n)])); });
 }
 
-// sin and cos of a phase of up to a few hundred radians: exact two-constant reduction to r = x/(2 pi) - k in
-// [-1/2, 1/2] revolutions, then the SFU (sin.approx / cos.approx on [-pi, pi]: absolute error ~4e-7, which the
-// images see as a relative error of the same size; DESIGN.md section 5 "precision budget").
-__device__ __forceinline__ void sincos_reduced(const float x, float* s, float* c)
-{
-    const float kInv2PiHi = 0.15915493667125702f, kInv2PiLo = 6.4206383266e-09f;
-    const float k = rintf(x * kInv2PiHi);
-    float r = fmaf(x, kInv2PiHi, -k);
-    r = fmaf(x, kInv2PiLo, r);
-    const float a = r * 6.283185307179586f;
-    *s = __sinf(a);
-    *c = __cosf(a);
-}
-
 struct WorkItem { int p, q0, cnt, pad; };
 
 struct FusedArgs {
