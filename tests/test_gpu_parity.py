@@ -295,3 +295,42 @@ def test_big_fft_sizes_ngs_sensor_and_psf(n_sub, psf_fft, n_steps):
         assert rel_l2(p[di].cpu().numpy(), ref["psf"][s]) <= IMAGE_TOL
         assert rel_l2(p2[di].cpu().numpy(), 2.0 * ref["psf"][s]) <= IMAGE_TOL
         assert abs(float(p[di].sum()) / n_steps - 1.0) < 1e-4          # Parseval: every PSF sums to 1
+
+
+def _fused_vs_oracle(cfg, n_steps, step0):
+    import torch
+    ref = oracle.forward(cfg, step0, n_steps)
+    geo = _geo(cfg, n_steps)
+    img, slp = geo.sh_images(0, None, step0, n_steps, cfg.dt_s)
+    torch.cuda.synchronize()
+    return check_wfs(cfg, geo, ref, 0, img, slp, n_steps, cfg.name)
+
+
+def test_fused_two_step_tiles_odd_counts_and_offsets():
+    """The fused kernel pairs consecutive steps per CTA: odd step counts, odd first steps and a single
+    step must give the same results as the oracle (the unpaired last step is computed but not stored)."""
+    for n_steps, step0 in ((1, 0), (1, 7), (3, 1), (5, 498)):
+        cfg = inputs.make_config(2, n_sub=9, screen_n=512, n_steps=n_steps)
+        _fused_vs_oracle(cfg, n_steps, step0)
+
+
+def test_fused_large_wind_shift_between_paired_steps():
+    """Wind of 300 m/s: the two steps of a pair are 15 screen pixels apart, the staged box is their union
+    (and wraps the periodic screen edge many times over 40 steps)."""
+    cfg = inputs.make_config(2, n_sub=9, screen_n=512, n_steps=2)
+    for i, lay in enumerate(cfg.layers):
+        lay.wind_x_mps, lay.wind_y_mps = (300.0, -250.0) if i % 2 else (-280.0, 310.0)
+    _fused_vs_oracle(cfg, 2, 39)
+
+
+def test_low_altitude_source_falls_back_to_generic_path():
+    """A beacon at 30 km under 25 km of turbulence compresses the top layers to du = gamma d_s/d_l < 1/2,
+    outside the row march of the fused kernel (1/2 <= du <= 1): the library must take the generic
+    trace + SH path and still match the oracle."""
+    cfg = inputs.make_config(2, n_sub=9, screen_n=512, n_steps=2)
+    for s in cfg.sources:
+        s.altitude_m = 30e3
+    _fused_vs_oracle(cfg, 2, 3)
+    out = _run_all(cfg, 2, 3)
+    ref = oracle.forward(cfg, 3, 2)
+    _check_phase(cfg, out["geo"], out["phase"], ref, 2)
