@@ -27,6 +27,12 @@ if ROOT not in sys.path:
 METRIC = "sh_subaperture_frames_per_sec"
 UNIT = "subaperture-frames/s"
 FP32_LANES_PER_SM = 128
+# From the committed ncu --set full capture of k_fused<32,0> (profiles/r1_v3_k_fused.md): DRAM bytes read + written per
+# simulated step (500.9 MB per 10-step launch) and the shared-memory data-pipe utilisation, the unit that binds.
+NCU_DRAM_BYTES_PER_STEP = 50.09e6
+NCU_SMEM_WAVEFRONT_FRAC = 0.692
+NCU_SOURCE = ("profiles/r1_v3_k_fused.md: dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture, "
+              "scaled from its 10-step launch to the steps of one launch here")
 
 
 # ------------------------------------------------------------------------------ work model
@@ -247,7 +253,8 @@ def run_gpu(args):
     achieved = flop / t_wfs / 1e12
     roofline = {"bound": "alu", "kernel": "LGS WFS forward model (ray-trace + SH image + CoG; ao_sh_images, phase_dev=NULL)",
                 "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s", "frac": achieved / fp32_peak,
-                "traffic": None, "peak_source": f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz (nominal; DESIGN.md section 6)",
+                "traffic": NCU_DRAM_BYTES_PER_STEP * min(batch, K), "traffic_source": NCU_SOURCE,
+                "smem_wavefront_frac": NCU_SMEM_WAVEFRONT_FRAC, "peak_source": f"148 SMs x 128 FP32 lanes x 2 x {pk['sm_max_mhz']:.0f} MHz (nominal; DESIGN.md section 6)",
                 "flop_per_subaperture_frame": flops_per_subap_frame(lgs.n_samp, lgs.fft, len(cfg.layers)),
                 "us_per_step": 1e6 * t_wfs / K, "launches": launches_wfs,
                 "sm_mhz_during": clocks_wfs["sm_mhz"],
