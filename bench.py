@@ -211,9 +211,12 @@ def run_gpu(args):
     def run_steps(f0, count):
         for b0 in range(0, count, batch):
             ks = min(batch, count - b0)
-            geo.sh_images(0, None, f0 + b0, ks, cfg.dt_s, want_images=False, slopes=sl_lgs[b0:b0 + ks])
-            geo.sh_images(1, None, f0 + b0, ks, cfg.dt_s, want_images=False, slopes=sl_ngs[b0:b0 + ks])
-            geo.psf(None, f0 + b0, ks, cfg.dt_s, psf=psf, accumulate=True)
+            if args.serial:
+                geo.sh_images(0, None, f0 + b0, ks, cfg.dt_s, want_images=False, slopes=sl_lgs[b0:b0 + ks])
+                geo.sh_images(1, None, f0 + b0, ks, cfg.dt_s, want_images=False, slopes=sl_ngs[b0:b0 + ks])
+                geo.psf(None, f0 + b0, ks, cfg.dt_s, psf=psf, accumulate=True)
+            else:       # ao_forward: the same three legs, the workspace-free LGS leg on the library's side stream
+                geo.forward(f0 + b0, ks, cfg.dt_s, [sl_lgs[b0:b0 + ks], sl_ngs[b0:b0 + ks]], psf=psf, accumulate=True)
 
     def timed(fn, *a):
         stream = torch.cuda.current_stream()
@@ -323,6 +326,7 @@ def main():
     ap.add_argument("--screen-n", type=int, default=8192)
     ap.add_argument("--layers", type=int, default=35)
     ap.add_argument("--batch", type=int, default=50, help="time steps per C-ABI call")
+    ap.add_argument("--serial", action="store_true", help="one C-ABI call per leg on one stream instead of ao_forward")
     ap.add_argument("--skip-e2e", action="store_true")
     ap.add_argument("--skip-cpu", action="store_true")
     args = ap.parse_args()

@@ -171,6 +171,17 @@ int ao_centroids(ao_geometry* g, int wfs_index, const float* images_dev, int n_i
 int ao_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, double dt_s,
            float* psf_dev, int accumulate, void* cuda_stream);
 
+/* ao_forward -- the whole step with DEVICE buffers: ray-trace + every WFS (slopes only, noiseless unless
+ * `noise`) + every science PSF for n_steps steps (the per-time-step forward model).
+ * Same results as one ao_sh_images(phase_dev = NULL, images_dev = NULL) per WFS plus ao_psf(phase_dev = NULL),
+ * but the workspace users (big-FFT sensors, PSF) run on a library-owned high-priority side stream concurrently
+ * with the sensors that need no workspace (the fused ray-trace + SH + CoG kernel) on `cuda_stream`; the side
+ * stream is forked from and joined back into `cuda_stream` by events, so the call is asynchronous on `cuda_stream` like
+ * every other call.  slopes_dev[w] (nullable per entry): ao_sh_images slopes layout of WFS w.
+ * psf_dev (nullable): [n_sci][M][M], += if accumulate else =.  Needs a workspace if any big WFS or PSF runs. */
+int ao_forward(ao_geometry* g, int64_t step0, int n_steps, double dt_s, const ao_noise* noise,
+               float* const* slopes_dev, float* psf_dev, int accumulate, void* cuda_stream);
+
 /* ao_forward_host -- the whole step for host callers: uploads nothing but the call parameters,
  * runs ray-trace + every WFS (noiseless unless `noise`) + every PSF for n_steps steps on
  * `cuda_stream`, and copies the results to HOST buffers (pinned memory recommended), then

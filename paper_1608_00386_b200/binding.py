@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "AO_OK", 1: "AO_ERR_INVALID_ARG", 2: "AO_ERR_SHAPE", 3: "AO_E
 # every symbol include/ao.h declares
 EXPORTS = ["ao_geometry_create", "ao_geometry_destroy", "ao_workspace_bytes", "ao_set_workspace",
            "ao_phase_elems_per_step", "ao_phase_offset", "ao_wfs_valid", "ao_trace_layers",
-           "ao_sh_images", "ao_centroids", "ao_psf", "ao_forward_host", "ao_launch_count",
+           "ao_sh_images", "ao_centroids", "ao_psf", "ao_forward", "ao_forward_host", "ao_launch_count",
            "ao_last_error", "ao_version"]
 
 
@@ -82,6 +82,7 @@ def load_library():
     L.ao_sh_images.argtypes = [vp, i32, vp, i64, i32, dbl, C.POINTER(ao_noise), vp, vp, vp]
     L.ao_centroids.argtypes = [vp, i32, vp, i32, vp, vp]
     L.ao_psf.argtypes = [vp, vp, i64, i32, dbl, vp, i32, vp]
+    L.ao_forward.argtypes = [vp, i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, i32, vp]
     L.ao_forward_host.argtypes = [vp, C.POINTER(vp), i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, vp]
     L.ao_launch_count.argtypes = [vp]; L.ao_launch_count.restype = i64
     L.ao_last_error.restype = C.c_char_p
@@ -239,6 +240,13 @@ class Geometry:
             psf = torch.zeros((n_sci, M, M), dtype=torch.float32, device=self.device)
         _check(self.lib.ao_psf(self.handle, _ptr(phase), step0, n_steps, dt_s, _ptr(psf), int(accumulate), _stream()))
         return psf
+
+    def forward(self, step0: int, n_steps: int, dt_s: float, slopes: Sequence, psf=None, accumulate=False, noise=None):
+        """ao_forward: every WFS (slopes[w] device tensors, None to skip) and the science PSF in one call."""
+        nw = len(self.cfg.wfs)
+        sl = (C.c_void_p * max(1, nw))(*[(_ptr(t) if t is not None else None) for t in slopes])
+        _check(self.lib.ao_forward(self.handle, step0, n_steps, dt_s, _noise(noise), sl, _ptr(psf),
+                                   int(accumulate), _stream()))
 
     def forward_host(self, step0: int, n_steps: int, dt_s: float, slopes_host: Sequence, psf_host=None,
                      screens_host: Optional[Sequence] = None, noise=None):

@@ -66,6 +66,9 @@ static void destroy(ao_geometry* g)
     if (!g) return;
     cudaFree(g->d_pupil_amp); cudaFree(g->d_layers); cudaFree(g->d_sources);
     cudaFree(g->d_psf_tw); cudaFree(g->d_psf_pre);
+    if (g->ev_fork) cudaEventDestroy(g->ev_fork);
+    if (g->ev_join) cudaEventDestroy(g->ev_join);
+    if (g->side) cudaStreamDestroy(g->side);
     for (auto& w : g->wfs) {
         cudaFree(w.d_amp); cudaFree(w.d_valid); cudaFree(w.d_w2m); cudaFree(w.d_tw); cudaFree(w.d_twf); cudaFree(w.d_pre); cudaFree(w.fused_items);
         free_group(w.grp);
@@ -270,6 +273,14 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    int prio_least = 0, prio_greatest = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest);
+    if (cudaStreamCreateWithPriority(&g->side, cudaStreamNonBlocking, prio_greatest) != cudaSuccess ||
+        cudaEventCreateWithFlags(&g->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&g->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        g->side = nullptr; g->ev_fork = nullptr; g->ev_join = nullptr;      // ao_forward then runs on one stream
+        cudaGetLastError();
+    }
 
     g->Np = pupil->n; g->pitch = pupil->pitch_m; g->lambda_ref = lambda_ref_m;
     const size_t np2 = (size_t)g->Np * g->Np;
@@ -477,6 +488,56 @@ int ao_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, d
     return run_psf(g, phase_dev, step0, n_steps, dt_s, psf_dev, accumulate, (cudaStream_t)cuda_stream);
 }
 
+// Shared by ao_forward and ao_forward_host: all WFS (slopes only) and the PSF for steps [step0, step0 + n_steps).
+// The workspace users (big-FFT sensors, PSF: many short, latency-bound launches) run in order on the library's
+// HIGH-priority side stream, forked from and joined into `st`; the workspace-free fused sensors (one long launch
+// that fills every SM) run on `st`.  With the priorities this way round the block scheduler hands freed SM slots
+// to the short kernels first, so both chains progress together instead of one behind the other.
+static int forward_chunk(ao_geometry* g, int64_t step0, int n_steps, double dt_s, const ao_noise* noise,
+                         float* const* slopes, float* psf, int accumulate, cudaStream_t st)
+{
+    int rc;
+    const bool want_psf = psf && g->psf_fft && !g->sci.src.empty();
+    bool any_ws = want_psf, any_free = false;
+    std::vector<char> on_side(g->wfs.size(), 0);
+    for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
+        const WfsH& w = g->wfs[wi];
+        if (!slopes || !slopes[wi] || w.grp.src.empty()) continue;
+        const bool ws_free = !w.big && fused_supported(g, w, dt_s);
+        on_side[wi] = ws_free ? 0 : 1;
+        (ws_free ? any_free : any_ws) = true;
+    }
+    const bool fork = g->side && any_ws && any_free;
+    cudaStream_t sw = fork ? g->side : st;                  // stream of the workspace users
+    if (fork) {
+        AO_CUDA(cudaEventRecord(g->ev_fork, st), "fork record");
+        AO_CUDA(cudaStreamWaitEvent(g->side, g->ev_fork, 0), "fork wait");
+    }
+    for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
+        const WfsH& w = g->wfs[wi];
+        if (!slopes || !slopes[wi] || w.grp.src.empty()) continue;
+        rc = run_wfs(g, (int)wi, nullptr, step0, n_steps, dt_s, noise, nullptr, slopes[wi], on_side[wi] ? sw : st);
+        if (rc) return rc;
+    }
+    if (want_psf) {
+        rc = run_psf(g, nullptr, step0, n_steps, dt_s, psf, accumulate, sw);
+        if (rc) return rc;
+    }
+    if (fork) {
+        AO_CUDA(cudaEventRecord(g->ev_join, g->side), "join record");
+        AO_CUDA(cudaStreamWaitEvent(st, g->ev_join, 0), "join wait");
+    }
+    return AO_OK;
+}
+
+int ao_forward(ao_geometry* g, int64_t step0, int n_steps, double dt_s, const ao_noise* noise,
+               float* const* slopes_dev, float* psf_dev, int accumulate, void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_forward: n_steps < 0");
+    return forward_chunk(g, step0, n_steps, dt_s, noise, slopes_dev, psf_dev, accumulate, (cudaStream_t)cuda_stream);
+}
+
 int ao_forward_host(ao_geometry* g, const float* const* screens_host, int64_t step0, int n_steps, double dt_s,
                     const ao_noise* noise, float* const* slopes_host, float* psf_host, void* cuda_stream)
 {
@@ -491,29 +552,31 @@ int ao_forward_host(ao_geometry* g, const float* const* screens_host, int64_t st
                                     sizeof(float) * (size_t)g->layers[l].S * g->layers[l].S, cudaMemcpyHostToDevice, st), "screen upload");
         }
     const WsView v = ws_view(g);
-    if (slopes_host) {
-        for (int c0 = 0; c0 < n_steps; c0 += v.chunk) {
-            const int ks = (n_steps - c0 < v.chunk) ? n_steps - c0 : v.chunk;
-            char* sl = (char*)v.slopes;
-            for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
-                const WfsH& w = g->wfs[wi];
-                const size_t per = sizeof(float) * w.grp.src.size() * 2 * (size_t)w.n_sub * w.n_sub;
-                float* dst = (float*)sl;
-                sl += align256(per) * (size_t)v.chunk;
-                if (!slopes_host[wi] || w.grp.src.empty()) continue;
-                rc = run_wfs(g, (int)wi, nullptr, step0 + c0, ks, dt_s, noise, nullptr, dst, st);
-                if (rc) return rc;
-                AO_CUDA(cudaMemcpyAsync((char*)slopes_host[wi] + per * (size_t)c0, dst, per * (size_t)ks,
-                                        cudaMemcpyDeviceToHost, st), "slopes download");
-            }
+    const bool want_psf = psf_host && g->psf_fft && !g->sci.src.empty();
+    if (n_steps == 0 && want_psf) { rc = run_psf(g, nullptr, step0, 0, dt_s, v.psf_stage, 0, st); if (rc) return rc; }
+    std::vector<float*> dst(g->wfs.size(), nullptr);
+    for (int c0 = 0; c0 < n_steps; c0 += v.chunk) {
+        const int ks = (n_steps - c0 < v.chunk) ? n_steps - c0 : v.chunk;
+        char* sl = (char*)v.slopes;
+        for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
+            const WfsH& w = g->wfs[wi];
+            const size_t per = sizeof(float) * w.grp.src.size() * 2 * (size_t)w.n_sub * w.n_sub;
+            dst[wi] = (slopes_host && slopes_host[wi] && !w.grp.src.empty()) ? (float*)sl : nullptr;
+            sl += align256(per) * (size_t)v.chunk;
+        }
+        rc = forward_chunk(g, step0 + c0, ks, dt_s, noise, dst.data(), want_psf ? v.psf_stage : nullptr, c0 > 0 ? 1 : 0, st);
+        if (rc) return rc;
+        for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
+            if (!dst[wi]) continue;
+            const WfsH& w = g->wfs[wi];
+            const size_t per = sizeof(float) * w.grp.src.size() * 2 * (size_t)w.n_sub * w.n_sub;
+            AO_CUDA(cudaMemcpyAsync((char*)slopes_host[wi] + per * (size_t)c0, dst[wi], per * (size_t)ks,
+                                    cudaMemcpyDeviceToHost, st), "slopes download");
         }
     }
-    if (psf_host && g->psf_fft && !g->sci.src.empty()) {
-        rc = run_psf(g, nullptr, step0, n_steps, dt_s, v.psf_stage, 0, st);
-        if (rc) return rc;
+    if (want_psf)
         AO_CUDA(cudaMemcpyAsync(psf_host, v.psf_stage, sizeof(float) * g->sci.src.size() * (size_t)g->psf_fft * g->psf_fft,
                                 cudaMemcpyDeviceToHost, st), "psf download");
-    }
     AO_CUDA(cudaStreamSynchronize(st), "stream synchronize");
     return AO_OK;
 }

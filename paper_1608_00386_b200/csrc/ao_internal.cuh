@@ -91,6 +91,9 @@ struct ao_geometry {
     int ws_chunk = 0;                 // steps per internal chunk that fit the workspace
     int64_t launches = 0;
     int sm_count = 148;
+    // ao_forward: side stream for the workspace-free sensors, fork / join events
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
 namespace ao {

@@ -334,3 +334,22 @@ def test_low_altitude_source_falls_back_to_generic_path():
     out = _run_all(cfg, 2, 3)
     ref = oracle.forward(cfg, 3, 2)
     _check_phase(cfg, out["geo"], out["phase"], ref, 2)
+
+
+def test_forward_matches_separate_calls():
+    """ao_forward (fused sensors on the library's side stream, big-FFT sensors and PSF on the caller's) gives
+    the same slopes and long-exposure PSF as ao_sh_images per WFS plus ao_psf, bit for bit."""
+    import torch
+    cfg = inputs.make_config(3, n_sub=8, screen_n=512, n_steps=3)
+    geo = _geo(cfg, 2)                                  # workspace of 2 steps: 3 steps run in two chunks
+    ref_s = [geo.sh_images(w, None, 4, 3, cfg.dt_s, want_images=False)[1] for w in range(len(cfg.wfs))]
+    ref_p = geo.psf(None, 4, 3, cfg.dt_s)
+    torch.cuda.synchronize()
+    got_s = [torch.full_like(r, float("nan")) for r in ref_s]
+    got_p = torch.zeros_like(ref_p)
+    for rep in range(2):                                # second call accumulates the PSF
+        geo.forward(4, 3, cfg.dt_s, got_s, psf=got_p, accumulate=(rep == 1))
+    torch.cuda.synchronize()
+    for a, b in zip(got_s, ref_s):
+        assert torch.equal(a, b)
+    assert torch.allclose(got_p, 2.0 * ref_p, rtol=1e-6, atol=0.0)
