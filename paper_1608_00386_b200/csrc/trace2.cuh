@@ -219,14 +219,20 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
     const uint32_t tiles_s = smem_u32(tiles), w_s = smem_u32(Wt);
     const uint32_t pb = (uint32_t)pitch * 4u, tile_bytes = (uint32_t)tile_floats * 4u;
     const int dbg = A.dbg;
-    int stage = 0, pstage = 0;
-    uint32_t par = 0, ppar = 0;                // stage/parity of layer a and of layer a-1
+    int stage = 0;
+    uint32_t par = 0;                          // stage and parity of layer a
+    // Refill lag: at iteration a the producer refills the stage of layer a - lag with layer a - lag + ns.  With
+    // lag = 1 it would wait for the slowest warp to finish the layer it has just finished itself (a CTA-wide
+    // rendezvous every layer, measured as 22 % of all stall samples); with lag = 2 the stage being recycled was
+    // released a whole layer ago and the copy still has one full layer of compute to land.
+    const int lag = ns >= 3 ? 2 : 1;
     for (int a = 0; a < nact; ++a) {
-        // refill the stage that layer a-1 used, once every warp has released it.  The producer role rotates:
-        // a fixed producer warp lags by its issue + table time every layer and paces the whole CTA.
-        if (warp == (a & (NT / 32 - 1)) && a >= 1 && a - 1 + ns < nact) {     // producer role rotates over the warps
-            mbar_wait(&S.empty_bar[pstage], ppar);
-            issue(a - 1 + ns, pstage);
+        // the producer role rotates over the warps: a fixed producer warp would lag by its issue + table time
+        // every layer and pace the whole CTA
+        if (warp == (a & (NT / 32 - 1)) && a >= lag && a - lag + ns < nact && !(A.dbg & 8)) {
+            const int l = a - lag, m = l / ns;
+            mbar_wait(&S.empty_bar[l - m * ns], (uint32_t)(m & 1));
+            issue(l + ns, l - m * ns);
         }
         const LayerT& T = L[a];
         const u64 du64 = ((u64)(unsigned)T.du_hi << 32) | (u64)T.duf;
@@ -263,7 +269,6 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&S.empty_bar[stage]);
-        pstage = stage; ppar = par;
         if (++stage == ns) { stage = 0; par ^= 1u; }
     }
 }
