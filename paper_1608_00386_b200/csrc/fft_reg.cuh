@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <type_traits>
 
+#include "pk_tma.cuh"
+
 namespace ao {
 
 // ---- compile-time trigonometry and complex constants ----
@@ -70,6 +72,42 @@ __device__ __forceinline__ void fft_stage(float2 (&x)[N])
         x[j] = cmul_cis<-pos, HALF>(make_float2(a.x - c.x, a.y - c.y));      // * exp(-2 pi i pos/(2 HALF))
     });
     if constexpr (HALF > 1) fft_stage<N, HALF / 2>(x);
+}
+
+// Packed-complex variant of fft_stage (fft_reg.cuh): a complex number is one f32x2 register pair, so the
+// butterfly add and subtract are one FADD2 each; twiddle multiplications stay scalar.
+template <int NUM, int DEN>
+__device__ __forceinline__ u64 cmul_cis_pk(const u64 x)
+{
+    using W = Cis<NUM, DEN>;
+    if constexpr (W::q == 0) return x;
+    else { const float2 r = cmul_cis<NUM, DEN>(unpack2(x)); return pack2(r.x, r.y); }
+}
+template <int N, int HALF>
+__device__ __forceinline__ void fft_stage_pk(u64 (&x)[N])
+{
+    static_for<0, N / 2>([&](auto bi) {
+        constexpr int b = decltype(bi)::value;
+        constexpr int grp = b / HALF, pos = b % HALF, i = grp * 2 * HALF + pos, j = i + HALF;
+        const u64 a = x[i], c = x[j];
+        x[i] = add2(a, c);
+        x[j] = cmul_cis_pk<-pos, HALF>(sub2(a, c));                            // * exp(-2 pi i pos/(2 HALF))
+    });
+    if constexpr (HALF > 1) fft_stage_pk<N, HALF / 2>(x);
+}
+
+// fft_stage on a float2 array through the packed butterflies (R-point DFT of the big-FFT passes).
+template <int N>
+__device__ __forceinline__ void fft_full_pk(float2 (&x)[N])
+{
+    if constexpr (N > 1) {
+        u64 y[N];
+#pragma unroll
+        for (int i = 0; i < N; ++i) y[i] = pack2(x[i].x, x[i].y);
+        fft_stage_pk<N, N / 2>(y);
+#pragma unroll
+        for (int i = 0; i < N; ++i) x[i] = unpack2(y[i]);
+    }
 }
 
 }  // namespace ao

@@ -63,7 +63,7 @@ __device__ __forceinline__ void pass_compute(const int tb, float2 (&v)[16], cons
 #pragma unroll
             for (int k = 1; k < R; ++k) x[k] = cmulf(x[k], __ldg(tw + t0 * k));
         }
-        if constexpr (R > 1) fft_stage<R, R / 2>(x);
+        fft_full_pk<R>(x);
         const int o = (b / NS) * (NS * R) + (b & (NS - 1));
 #pragma unroll
         for (int k = 0; k < R; ++k) st(o + k * NS, x[bitrev_c(k, R)], q * R + k);
@@ -106,7 +106,7 @@ struct BigRowArgs {
 
 // Pass 1.  grid (ceil(n / rows per CTA), batch), batch index b = (step * n_sel + si) * n_sub^2 + sa.
 template <int LOGM>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 k_big_rows(const BigRowArgs A)
 {
     using K = BigCfg<LOGM>;

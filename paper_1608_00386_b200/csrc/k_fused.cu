@@ -36,28 +36,6 @@ namespace ao {
 // First DIF stage on the half-zero input: X[2k'] = FFT_n(e[a] cis(pi (M-1) a/M))[k'],
 //                                         X[2k'+1] = FFT_n(e[a] cis(pi (M-3) a/M))[k'].
 // `sink(k, value)` is called once for every k (k as std::integral_constant).
-// Packed-complex variant of fft_stage (fft_reg.cuh): a complex number is one f32x2 register pair, so the
-// butterfly add and subtract are one FADD2 each; twiddle multiplications stay scalar.
-template <int NUM, int DEN>
-__device__ __forceinline__ u64 cmul_cis_pk(const u64 x)
-{
-    using W = Cis<NUM, DEN>;
-    if constexpr (W::q == 0) return x;
-    else { const float2 r = cmul_cis<NUM, DEN>(unpack2(x)); return pack2(r.x, r.y); }
-}
-template <int N, int HALF>
-__device__ __forceinline__ void fft_stage_pk(u64 (&x)[N])
-{
-    static_for<0, N / 2>([&](auto bi) {
-        constexpr int b = decltype(bi)::value;
-        constexpr int grp = b / HALF, pos = b % HALF, i = grp * 2 * HALF + pos, j = i + HALF;
-        const u64 a = x[i], c = x[j];
-        x[i] = add2(a, c);
-        x[j] = cmul_cis_pk<-pos, HALF>(sub2(a, c));                            // * exp(-2 pi i pos/(2 HALF))
-    });
-    if constexpr (HALF > 1) fft_stage_pk<N, HALF / 2>(x);
-}
-
 template <int M, typename Sink>
 __device__ __forceinline__ void dft_half_padded(const float2 (&e)[M / 2], Sink&& sink)
 {
