@@ -166,12 +166,50 @@ k_centroid(const float* __restrict__ images, const uint8_t* __restrict__ valid, 
     }
 }
 
+// Large detectors (the 128 x 128 images of the big-FFT sensors): one CTA per image, row-wise partial sums.
+__global__ void __launch_bounds__(256)
+k_centroid_big(const float* __restrict__ images, const uint8_t* __restrict__ valid, int nsa, int P,
+               float* __restrict__ slopes)
+{
+    __shared__ float red[3][8];
+    const long long img = blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long set = img / nsa;
+    const int sa = (int)(img - set * nsa);
+    const float* pimg = images + (size_t)img * P * P;
+    const float h = 0.5f * (float)(P - 1);
+    float s = 0.0f, mx = 0.0f, my = 0.0f;
+    for (int r = warp; r < P; r += 8) {                       // a warp per detector row
+        float rs = 0.0f;
+        for (int c = lane; c < P; c += 32) {
+            const float v = pimg[(size_t)r * P + c];
+            rs += v; mx = fmaf((float)c - h, v, mx);
+        }
+        s += rs; my = fmaf((float)r - h, rs, my);
+    }
+    s = warp_sum(s); mx = warp_sum(mx); my = warp_sum(my);
+    if (lane == 0) { red[0][warp] = s; red[1][warp] = mx; red[2][warp] = my; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        s = 0.0f; mx = 0.0f; my = 0.0f;
+        for (int w = 0; w < 8; ++w) { s += red[0][w]; mx += red[1][w]; my += red[2][w]; }
+        const bool ok = valid[sa] && fabsf(s) >= 1e-12f;
+        slopes[(size_t)(set * 2 + 0) * nsa + sa] = ok ? mx / s : 0.0f;
+        slopes[(size_t)(set * 2 + 1) * nsa + sa] = ok ? my / s : 0.0f;
+    }
+}
+
 cudaError_t launch_centroids(ao_geometry* g, const WfsH& w, const float* images, int n_sets,
                              float* slopes, cudaStream_t st)
 {
     const int nsa = w.n_sub * w.n_sub;
     const long long n_img = (long long)n_sets * nsa;
     if (n_img <= 0) return cudaSuccess;
+    if (w.P >= 64 && n_img <= 0x7fffffffLL) {
+        k_centroid_big<<<(unsigned)n_img, 256, 0, st>>>(images, w.d_valid, nsa, w.P, slopes);
+        g->launches++;
+        return cudaGetLastError();
+    }
     const long long blocks = (n_img + 7) / 8;
     k_centroid<<<(unsigned)blocks, 256, 0, st>>>(images, w.d_valid, nsa, w.P, n_img, slopes);
     g->launches++;
