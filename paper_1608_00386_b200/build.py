@@ -39,6 +39,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc] + NVCC_FLAGS + ["-I", os.path.join(ROOT, "include"), "-I", CSRC]
+    if os.environ.get("AO_BUILD_PROFILE"):       # component-timing switches (AO_DBG) for profiling, never for results
+        cmd += ["-DAO_PROFILE_SWITCHES"]
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += sources() + ["-o", LIB]

@@ -63,7 +63,10 @@ inline Trace2Args make_trace2_args(const ao_geometry* g, const Tile2Plan& pl, in
     Trace2Args t;
     t.layers = g->d_layers; t.n_layers = (int)g->layers.size(); t.srcs = g->d_sources;
     t.step0 = (long long)step0; t.dt = dt; t.pitch = pl.pitch; t.rows = pl.rows; t.ns = pl.ns;
+    t.dbg = 0;
+#ifdef AO_PROFILE_SWITCHES      // profiling builds only (AO_BUILD_PROFILE=1): switch parts of the kernel off, results are wrong
     { const char* ev = getenv("AO_DBG"); t.dbg = ev ? atoi(ev) : 0; }
+#endif
     return t;
 }
 
