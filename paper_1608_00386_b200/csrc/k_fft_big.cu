@@ -154,7 +154,9 @@ struct BigColArgs {
 
 // Pass 2.  MODE 0 (PSF): grid (M / C, n_dir); the CTA loops over the ks steps of the chunk.
 //          MODE 1 (SH):  grid (P, batch), C = beta, columns k0 + g beta .. of the detector window.
-template <int LOGM, int MODE>
+// CT: columns per CTA as a compile-time constant (0 = run-time A.C): with it every shared-memory index of the
+// Stockham passes is a per-thread base plus an immediate instead of a multiply per point.
+template <int LOGM, int MODE, int CT>
 __global__ void __launch_bounds__(MODE == 0 ? 512 : 1024)
 k_big_cols(const BigColArgs A)
 {
@@ -162,7 +164,7 @@ k_big_cols(const BigColArgs A)
     constexpr int M = K::M;
     extern __shared__ float4 smem_raw[];
     float2* sm = reinterpret_cast<float2*>(smem_raw);
-    const int tid = threadIdx.x, C = A.C, tb = tid / C, c = tid - tb * C;
+    const int tid = threadIdx.x, C = CT ? CT : A.C, tb = tid / C, c = tid - tb * C;
     const int n = A.n, g = blockIdx.x;
     const long long b = blockIdx.y;
     if (MODE == 0) {
@@ -275,15 +277,23 @@ static cudaError_t launch_rows_t(const BigRowArgs& a, int n_rows, unsigned batch
     return cudaGetLastError();
 }
 
-template <int LOGM, int MODE>
-static cudaError_t launch_cols_t(const BigColArgs& a, unsigned gx, unsigned gy, cudaStream_t st)
+template <int LOGM, int MODE, int CT>
+static cudaError_t launch_cols_ct(const BigColArgs& a, unsigned gx, unsigned gy, cudaStream_t st)
 {
     using K = BigCfg<LOGM>;
     const size_t smem = sizeof(float2) * (size_t)a.C * K::PADM;
-    cudaError_t e = cudaFuncSetAttribute(k_big_cols<LOGM, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_big_cols<LOGM, MODE, CT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_big_cols<LOGM, MODE><<<dim3(gx, gy), K::T * a.C, smem, st>>>(a);
+    k_big_cols<LOGM, MODE, CT><<<dim3(gx, gy), K::T * a.C, smem, st>>>(a);
     return cudaGetLastError();
+}
+
+template <int LOGM, int MODE>
+static cudaError_t launch_cols_t(const BigColArgs& a, unsigned gx, unsigned gy, cudaStream_t st)
+{
+    constexpr int CFAST = MODE == 0 ? 4 : 8;               // PSF at M >= 512 uses 4 columns, the NGS sensors bin 8 x 8
+    if (a.C == CFAST) return launch_cols_ct<LOGM, MODE, CFAST>(a, gx, gy, st);
+    return launch_cols_ct<LOGM, MODE, 0>(a, gx, gy, st);
 }
 
 #define AO_BIG_DISPATCH(logM, CALL)                                   \
