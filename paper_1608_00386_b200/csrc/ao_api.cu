@@ -101,7 +101,8 @@ static Plan make_plan(const ao_geometry* g)
         if ((size_t)w.grp.stage_elems > stage_elems) stage_elems = (size_t)w.grp.stage_elems;
         p.slopes += align256(sizeof(float) * n_sel * 2 * nsa);
         if (w.big) {
-            const size_t s = sh_big_scratch_bytes(g, w);
+            size_t s = sh_big_scratch_bytes(g, w);
+            if (2 * s <= ((size_t)96 << 20)) s *= 2;         // two steps per launch pair while the intermediate fits L2
             if (s > p.scratch) p.scratch = s;
             const size_t im = align256(sizeof(float) * n_sel * nsa * w.P * w.P);
             if (im > p.bigimg) p.bigimg = im;
@@ -182,7 +183,7 @@ static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0
             AO_CUDA(launch_sh_small(g, w, ph, api, stride, step0 + c0, ks, nz, img, slp, st), "sh_small");
         } else {
             float* im = img ? img : v.bigimg;
-            AO_CUDA(launch_sh_big(g, w, ph, api, stride, ks, v.scratch, im, st), "sh_big");
+            AO_CUDA(launch_sh_big(g, w, ph, api, stride, ks, v.scratch, make_plan(g).scratch, im, st), "sh_big");
             if (nz.on) AO_CUDA(launch_noise(g, w, im, step0 + c0, ks, nz, st), "noise");
             if (slp) AO_CUDA(launch_centroids(g, w, im, ks * (int)n_sel, slp, st), "centroids");
         }

@@ -115,7 +115,7 @@ cudaError_t launch_noise(ao_geometry* g, const WfsH& w, float* images, int64_t s
 // big FFT: SH mode for one step-chunk of WFS w (images out); PSF mode for ks <= psf_chunk_steps(g)
 // consecutive steps summed into psf (phase of step j at phase + j * step_stride).
 cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, bool api_layout,
-                          long long step_stride, int n_steps, float2* scratch, float* images,
+                          long long step_stride, int n_steps, float2* scratch, size_t scratch_bytes, float* images,
                           cudaStream_t st);
 cudaError_t launch_psf(ao_geometry* g, const float* phase, bool api_layout, long long step_stride,
                        int ks, float2* scratch, float* psf, int accumulate, cudaStream_t st);

@@ -16,6 +16,8 @@
 //   - PSF: accumulates the steps of a chunk in registers and adds them to the long exposure once;
 //   - SH: sums the beta x beta detector bins (C = beta: one detector column per CTA).
 // The scratch of a chunk stays L2-resident between the two passes.
+#include <algorithm>
+
 #include "ao_device.cuh"
 #include "fft_reg.cuh"
 
@@ -326,7 +328,7 @@ cudaError_t launch_sh_big_generic(ao_geometry* g, const WfsH& w, const float* ph
                                   cudaStream_t st);
 
 cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, bool api_layout,
-                          long long step_stride, int n_steps, float2* scratch, float* images,
+                          long long step_stride, int n_steps, float2* scratch, size_t scratch_bytes, float* images,
                           cudaStream_t st)
 {
     if (!sh_big_fast(w)) return launch_sh_big_generic(g, w, phase, api_layout, step_stride, n_steps, scratch, images, st);
@@ -334,14 +336,19 @@ cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, boo
     if (n_sel == 0 || n_steps <= 0) return cudaSuccess;
     cudaError_t e;
     const unsigned batch = (unsigned)(n_sel * nsa);
-    // one step at a time: the scratch holds one step of this WFS
-    for (int k = 0; k < n_steps; ++k) {
+    // as many steps per launch pair as the scratch holds (at most 4: the intermediate should stay inside L2)
+    const size_t per_step = sh_big_scratch_bytes(g, w);
+    int kb = per_step ? (int)std::min<size_t>(4, scratch_bytes / per_step) : 1;
+    if (kb < 1) kb = 1;
+    while (kb > 1 && (size_t)kb * per_step > ((size_t)96 << 20)) --kb;
+    for (int k = 0; k < n_steps; k += kb) {
+        const int kn = n_steps - k < kb ? n_steps - k : kb;
         BigRowArgs r;
         r.phase = phase + (size_t)k * step_stride; r.step_stride = step_stride;
         r.off = api_layout ? w.grp.d_off_api : w.grp.d_off_stage; r.n_sel = n_sel;
         r.amp = w.d_amp; r.valid = w.d_valid; r.n_sub = w.n_sub; r.n = w.n;
         r.tw = w.d_twf; r.pre = w.d_pre; r.T = scratch;
-        if ((e = launch_rows(w.logM, r, w.n, batch, st)) != cudaSuccess) return e;
+        if ((e = launch_rows(w.logM, r, w.n, batch * (unsigned)kn, st)) != cudaSuccess) return e;
         g->launches++;
         BigColArgs c;
         c.T = scratch; c.valid = w.d_valid; c.nsa = nsa; c.n = w.n; c.C = w.beta; c.tw = w.d_twf;
@@ -349,7 +356,7 @@ cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, boo
         c.beta = w.beta; c.P = w.P; c.k0 = (w.M - w.beta * w.P) / 2;
         c.n_dir = 1; c.ks = 1; c.accumulate = 0;
         c.out = images + (size_t)k * batch * w.P * w.P;
-        if ((e = launch_cols_sh(w.logM, c, (unsigned)w.P, batch, st)) != cudaSuccess) return e;
+        if ((e = launch_cols_sh(w.logM, c, (unsigned)w.P, batch * (unsigned)kn, st)) != cudaSuccess) return e;
         g->launches++;
     }
     return cudaSuccess;
