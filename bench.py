@@ -27,11 +27,11 @@ if ROOT not in sys.path:
 METRIC = "sh_subaperture_frames_per_sec"
 UNIT = "subaperture-frames/s"
 FP32_LANES_PER_SM = 128
-# From the committed ncu --set full capture of k_fused<32,0> (profiles/r1_v3_k_fused.md): DRAM bytes read + written per
-# simulated step (500.9 MB per 10-step launch) and the shared-memory data-pipe utilisation, the unit that binds.
-NCU_DRAM_BYTES_PER_STEP = 50.09e6
-NCU_SMEM_WAVEFRONT_FRAC = 0.692
-NCU_SOURCE = ("profiles/r1_v3_k_fused.md: dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture, "
+# From the committed ncu --set full capture of k_fused<32,0> (profiles/r1_v4_k_fused.md): DRAM bytes read + written per
+# simulated step (506.2 MB per 10-step launch) and the shared-memory data-pipe utilisation, the unit that binds.
+NCU_DRAM_BYTES_PER_STEP = 50.62e6
+NCU_SMEM_WAVEFRONT_FRAC = 0.735
+NCU_SOURCE = ("profiles/r1_v4_k_fused.md: dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture, "
               "scaled from its 10-step launch to the steps of one launch here")
 
 
