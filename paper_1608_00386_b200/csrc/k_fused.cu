@@ -82,7 +82,7 @@ struct FusedCfg {
     static_assert(kTR % n == 0 && NT % n == 0 && n <= 32, "bad fused configuration");
 };
 
-template <int M, bool NOISE>
+template <int M, bool NOISE, bool ANYDU>
 __global__ void __launch_bounds__(kFusedThreads, 4)
 k_fused(const FusedArgs A)
 {
@@ -104,7 +104,7 @@ k_fused(const FusedArgs A)
     // ---- phase A: ray-trace of the 16 x 256 tile, two steps, into registers ----
     u64 acc[kKS * kTR];
     double refsum[2];                                      // unused: |FFT|^2 is piston-invariant per subaperture
-    trace2_tile<NT, false>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, refsum);
+    trace2_tile<NT, false, ANYDU>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, refsum);
     __syncthreads();                                       // stages are dead: shared memory becomes the exchange buffer
 
     // ---- phase B: image formation, one (subaperture row, column slot) round at a time ----
@@ -239,7 +239,8 @@ template <int M>
 static cudaError_t launch_fused_variant(ao_geometry* g, const WfsH& w, FusedArgs a, const Tile2Plan& pl, int n_steps,
                                         cudaStream_t st)
 {
-    auto kern = a.nz.on ? k_fused<M, true> : k_fused<M, false>;
+    auto kern = pl.anydu ? (a.nz.on ? k_fused<M, true, true> : k_fused<M, false, true>)
+                         : (a.nz.on ? k_fused<M, true, false> : k_fused<M, false, false>);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     const size_t nsa = (size_t)w.n_sub * w.n_sub;

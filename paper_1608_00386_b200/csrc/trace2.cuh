@@ -44,7 +44,7 @@ struct __align__(16) LayerT {
     int cw, rw;           // start column / row of the staged box, wrapped into [0, S)
     int wt, rt;           // box width (multiple of 4) and rows
     unsigned duf;         // frac(du) 2^32
-    int du_hi;            // floor(du): 1 when du == 1
+    int du_hi;            // floor(du)
     int lay;              // layer index
     double du;            // screen pixels per output sample
     double vrel[kKS];     // row coordinate of tile row 0 relative to box row 0
@@ -96,6 +96,24 @@ __device__ __forceinline__ void t2_march(u64 (&acc)[kKS * kTR], const uint32_t t
     }
 }
 
+// The same for ANY du > 0 (screen pixels per output sample): every output row builds both its top and its bottom
+// x-interpolated row from eight taps, acc_i += w0 X[r_i] + w1 X[r_i + 1]; about 1.5 times the work of t2_march,
+// still one basic block.  Used when a layer falls outside 1/2 <= du <= 1 (c4 at M = 16: the WFS grid is coarser
+// than the screens, du up to 1.5; low beacons).  Table entry: (w0, w1, byte offset of X[r_i] relative to X[r_0]).
+template <int OFF>
+__device__ __forceinline__ void t2_march_any(u64 (&acc)[kKS * kTR], const uint32_t tp0, const uint32_t tp1, const uint32_t pb,
+                                             const u64 fx, const u64 ref, const uint32_t wtab)
+{
+#pragma unroll
+    for (int i = 0; i < kTR; ++i) {
+        const float4 w = lds_f32x4(wtab + 16u * (uint32_t)i);
+        const uint32_t off = __float_as_uint(w.z);
+        const u64 top = t2_xrow(tp0 + off, tp1 + off, fx, ref);
+        const u64 bot = t2_xrow(tp0 + off + pb, tp1 + off + pb, fx, ref);
+        acc[OFF + i] = fma2(pack2(w.y, w.y), bot, fma2(pack2(w.x, w.x), top, acc[OFF + i]));
+    }
+}
+
 // Ray-trace one tile for two steps: rows ifirst .. ifirst+15, columns jfirst + {tid, tid + NT} of source `sp` at
 // time steps step_first and step_first + 1.  acc[s * 16 + i] receives the packed (column tid, column tid + NT)
 // layer sums of step s, row i, minus warp-uniform piston references (the same for both steps); with REFSUM
@@ -103,7 +121,7 @@ __device__ __forceinline__ void t2_march(u64 (&acc)[kKS * kTR], const uint32_t t
 // `dyn`: dynamic shared memory, 128-byte aligned: [ns][rows][pitch] floats, then trace2_sched_bytes(n_layers).
 // All NT threads call it.  On return every thread has finished reading the stages, but other warps may not
 // have: __syncthreads() before reusing the memory.
-template <int NT, bool REFSUM>
+template <int NT, bool REFSUM, bool ANYDU>
 __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& sp, Trace2Shared& S, unsigned char* dyn,
                                             const int jfirst, const int ifirst, const long long step_first,
                                             u64 (&acc)[kKS * kTR], double (&refsum)[2])
@@ -160,7 +178,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         long long cw = cmin % lp.S; if (cw < 0) cw += lp.S;
         long long rw = rmin % lp.S; if (rw < 0) rw += lp.S;
         T.scr = lp.screen; T.S = lp.S; T.cw = (int)cw; T.rw = (int)rw; T.wt = wt; T.rt = rt;
-        T.du = du; T.du_hi = du >= 1.0 ? 1 : 0;
+        T.du = du; T.du_hi = (int)floor(du);
         const unsigned long long f = __double2ull_rn((du - (double)T.du_hi) * 4294967296.0);
         T.duf = f > 0xffffffffull ? 0xffffffffu : (unsigned)f;
 #pragma unroll
@@ -192,6 +210,12 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             }
             const double fy = v - (double)r;
             const float w0 = (float)(1.0 - fy);
+            if (ANYDU) {
+                const long long ru = (long long)floor(v);                       // unclamped: rows may advance by 2 or more
+                const double fu = v - (double)ru;
+                Wt[stage * (kKS * kTR) + lane] = make_float4((float)(1.0 - fu), (float)fu,
+                                                              __uint_as_float((uint32_t)((int)(ru - r0) * pitch * 4)), 0.0f);
+            } else
             Wt[stage * (kKS * kTR) + lane] = make_float4((float)fy, adv ? w0 : 0.0f, adv ? 0.0f : w0,
                                                           __uint_as_float((uint32_t)((int)(r + 1 - r0) * pitch * 4)));
             if (i == 0) R0[stage * kKS + s] = (int)r;
@@ -256,15 +280,19 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
                 const u64 U0 = uf0 + colA, U1 = uf0 + colB;
                 const u64 fx = pack2(__uint2float_rn((unsigned)U0) * k32, __uint2float_rn((unsigned)U1) * k32);
                 const uint32_t rowb = tile_s + (uint32_t)ro0 * pb;
-                t2_march<0>(acc, rowb + (uint32_t)(U0 >> 32) * 4u, rowb + (uint32_t)(U1 >> 32) * 4u, fx, ref,
-                            w_s + (uint32_t)(stage * kKS + 0) * (kTR * 16));
+                const uint32_t t0 = rowb + (uint32_t)(U0 >> 32) * 4u, t1 = rowb + (uint32_t)(U1 >> 32) * 4u;
+                const uint32_t wt_s = w_s + (uint32_t)(stage * kKS + 0) * (kTR * 16);
+                if (ANYDU) t2_march_any<0>(acc, t0, t1, pb, fx, ref, wt_s);
+                else t2_march<0>(acc, t0, t1, fx, ref, wt_s);
             }
             {
                 const u64 U0 = uf1 + colA, U1 = uf1 + colB;
                 const u64 fx = pack2(__uint2float_rn((unsigned)U0) * k32, __uint2float_rn((unsigned)U1) * k32);
                 const uint32_t rowb = tile_s + (uint32_t)ro1 * pb;
-                t2_march<kTR>(acc, rowb + (uint32_t)(U0 >> 32) * 4u, rowb + (uint32_t)(U1 >> 32) * 4u, fx, ref,
-                              w_s + (uint32_t)(stage * kKS + 1) * (kTR * 16));
+                const uint32_t t0 = rowb + (uint32_t)(U0 >> 32) * 4u, t1 = rowb + (uint32_t)(U1 >> 32) * 4u;
+                const uint32_t wt_s = w_s + (uint32_t)(stage * kKS + 1) * (kTR * 16);
+                if (ANYDU) t2_march_any<kTR>(acc, t0, t1, pb, fx, ref, wt_s);
+                else t2_march<kTR>(acc, t0, t1, fx, ref, wt_s);
             }
         }
         __syncwarp();

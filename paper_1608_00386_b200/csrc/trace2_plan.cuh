@@ -13,14 +13,14 @@ namespace ao {
 constexpr int kFusedThreads = 128;
 constexpr int kTileCols = 2 * kFusedThreads;
 
-struct Tile2Plan { bool ok; int pitch, rows, ns; size_t smem; };
+struct Tile2Plan { bool ok; int pitch, rows, ns; size_t smem; int anydu; };
 
 // Staging plan of the two-step tiled ray-trace for the sources `src` (all active layers): the union box of a
-// 16 x 256 tile over two consecutive steps must fit a shared-memory stage and the row march needs
-// 1/2 <= du <= 1 (screen pixels per output sample).  `min_bytes`: floor on the stage region (the exchange buffer of k_fused aliases it).
+// 16 x 256 tile over two consecutive steps must fit a shared-memory stage.  Layers with 1/2 <= du <= 1 (screen
+// pixels per output sample) take the three-term row march; if any layer is outside, the two-row march runs.  `min_bytes`: floor on the stage region (the exchange buffer of k_fused aliases it).
 inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, double dt, size_t min_bytes)
 {
-    Tile2Plan pl = {false, 0, 0, 0, 0};
+    Tile2Plan pl = {false, 0, 0, 0, 0, 0};
     double ext_x = 0.0, ext_y = 0.0;                               // box extent beyond the taps, screen pixels
     int s_min = 1 << 30;
     bool any = false;
@@ -30,7 +30,8 @@ inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, 
             if (!(lp.height < sp.H)) continue;
             double du = (1.0 - lp.height * sp.inv_H) * sp.d * lp.inv_pitch;
             if (fabs(du - 1.0) < 1e-9) du = 1.0;
-            if (!(du >= 0.5) || du > 1.0) return pl;             // the row march assumes 1/2 <= du <= 1
+            if (!(du > 0.0) || du > 8.0) return pl;               // absurd sampling ratio: not this path
+            if (du < 0.5 || du > 1.0) pl.anydu = 1;                // outside the three-term march: two-row march
             if (lp.S % 4 != 0) return pl;                          // 16-byte aligned rows for the bulk copies
             const double shx = fabs(lp.wx * dt * lp.inv_pitch) * (kKS - 1), shy = fabs(lp.wy * dt * lp.inv_pitch) * (kKS - 1);
             ext_x = std::max(ext_x, (kTileCols - 1) * du + shx);

@@ -323,10 +323,10 @@ def test_fused_large_wind_shift_between_paired_steps():
     _fused_vs_oracle(cfg, 2, 39)
 
 
-def test_low_altitude_source_falls_back_to_generic_path():
+def test_low_altitude_source_takes_the_two_row_march():
     """A beacon at 30 km under 25 km of turbulence compresses the top layers to du = gamma d_s/d_l < 1/2,
-    outside the row march of the fused kernel (1/2 <= du <= 1): the library must take the generic
-    trace + SH path and still match the oracle."""
+    outside the three-term row march (1/2 <= du <= 1): the fused kernel and the tiled phase writer must switch to
+    the two-row march (any du) and still match the oracle."""
     cfg = inputs.make_config(2, n_sub=9, screen_n=512, n_steps=2)
     for s in cfg.sources:
         s.altitude_m = 30e3
