@@ -120,6 +120,7 @@ cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, boo
 cudaError_t launch_psf(ao_geometry* g, const float* phase, bool api_layout, long long step_stride,
                        int ks, float2* scratch, float* psf, int accumulate, cudaStream_t st);
 int psf_chunk_steps(const ao_geometry* g);
+bool sh_big_fast(const WfsH& w);                                    // the Stockham two-pass path applies (else generic)
 
 // fused trace + SH + CoG (k_fused.cu); cudaErrorNotSupported if the geometry is outside its fast path
 bool fused_supported(const ao_geometry* g, const WfsH& w, double dt);

@@ -260,7 +260,7 @@ static int cols_threads_per_transform(int M) { return M / 16; }
 // The SH fast path needs C = beta columns per CTA: a power of two, full warps, at most 1024 threads.
 bool sh_big_fast(const WfsH& w)
 {
-    if (w.M < 128 || w.M > 4096 || (w.M & (w.M - 1))) return false;
+    if (w.M < 64 || w.M > 4096 || (w.M & (w.M - 1))) return false;
     const int T = cols_threads_per_transform(w.M), C = w.beta;
     if (C < 1 || C > 32 || (C & (C - 1))) return false;
     if (T * C < 32 || T * C > 1024 || w.P > 1024) return false;
