@@ -304,9 +304,9 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
         WfsH& w = g->wfs[i];
         w.n_sub = wfs[i].n_sub; w.n = wfs[i].n_samp; w.M = wfs[i].fft; w.beta = wfs[i].bin; w.P = wfs[i].n_pix;
         w.min_illum = wfs[i].min_illum; w.logM = ilog2(w.M);
-        // M > 64: two-pass HBM/L2 FFT.  M = 64 (c4's largest sweep point, n = 32: no fused kernel) takes it too when the
-        // Stockham passes apply and one step's subaperture frames fit a grid dimension; else the direct-DFT kernel.
-        w.big = w.M > 64 || (w.M == 64 && sh_big_fast(w) && (long long)w.n_sub * w.n_sub * n_src <= 65535);
+        // M > 64: two-pass HBM/L2 FFT.  M = 64 (c4's largest sweep point, n = 32: no fused kernel) is grouped with
+        // them: one CTA per subaperture with both passes in shared memory (k_sh_mid64), same tables, no scratch.
+        w.big = w.M >= 64;
         const int N = w.n_sub * w.n;
         const float* A = wfs[i].amp_host;
         w.valid.assign((size_t)w.n_sub * w.n_sub, 0);

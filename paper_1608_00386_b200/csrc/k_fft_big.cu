@@ -231,9 +231,96 @@ k_big_cols(const BigColArgs A)
     }
 }
 
+// ---- M = 64: the whole subaperture in one CTA -------------------------------------------------
+// One CTA of 256 threads per (step, source, subaperture): both passes of the 64 x 64 transform and the binning
+// stay in shared memory (no HBM scratch; the two-pass kernels above would move 16 KB per subaperture frame twice).
+// Pass A: the n non-zero rows, 4 threads per 64-point Stockham transform (64 transforms per CTA-wide call);
+// pass B: the 64 columns the same way, |.|^2 into shared memory; then beta x beta binning, 4 threads per pixel.
+struct MidArgs {
+    const float* phase; long long step_stride; const long long* off; int n_sel;
+    const float* amp; const uint8_t* valid; int n_sub, n;
+    const float2* tw; const float2* pre;
+    int beta, P, k0; float norm;
+    float* out;                                            // [batch][P][P]
+};
+
+__global__ void __launch_bounds__(256, 4)
+k_sh_mid64(const MidArgs A)
+{
+    using K = BigCfg<6>;
+    constexpr int M = 64, T = K::T, NTR = 256 / T, TP = M + 1;     // 64 transforms per pass, padded pitch
+    extern __shared__ float4 smem_raw[];
+    float2* sm = reinterpret_cast<float2*>(smem_raw);                // exchange buffer of the passes: [64][PADM]
+    float2* Tm = sm + NTR * K::PADM;                                 // row-pass output [n <= 64][TP] (n <= 32 used)
+    float* Ib = reinterpret_cast<float*>(Tm);                        // |.|^2 [M][TP], aliases Tm after pass B's loads
+    const int tid = threadIdx.x, r = tid / T, tb = tid - r * T;
+    const int n = A.n, nsa = A.n_sub * A.n_sub, P = A.P;
+    const long long b = blockIdx.x;
+    const int sa = (int)(b % nsa);
+    const long long set = b / nsa;
+    const int si = (int)(set % A.n_sel);
+    const long long k = set / A.n_sel;
+    float* out = A.out + (size_t)b * P * P;
+    if (A.valid && !A.valid[sa]) {                                   // CTA-uniform
+        for (int i = tid; i < P * P; i += 256) out[i] = 0.0f;
+        return;
+    }
+    const int p = sa / A.n_sub, q = sa - p * A.n_sub, N = A.n_sub * n;
+    {   // pass A: row r of the subaperture (rows >= n are zero and are not transformed: their output is unused)
+        const bool row_on = r < n;
+        const size_t rowoff = (size_t)(p * n + (row_on ? r : 0)) * N + (size_t)q * n;
+        const float* ph = A.phase + (size_t)k * A.step_stride + A.off[si] + rowoff;
+        const float* am = A.amp + rowoff;
+        const float2 pa = row_on ? A.pre[r] : make_float2(0.0f, 0.0f);
+        big_fft<6>(tb, sm, 1, r * K::PADM, A.tw,
+            [&](int i) {
+                float2 v = make_float2(0.0f, 0.0f);
+                if (row_on && i < n) {
+                    const float Am = __ldg(am + i);
+                    float s, c;
+                    sincos_reduced(__ldg(ph + i), &s, &c);
+                    v = cmulf(make_float2(Am * c, Am * s), cmulf(pa, __ldg(A.pre + i)));
+                }
+                return v;
+            },
+            [&](int i, const float2 x, int) { if (row_on) Tm[r * TP + i] = x; });
+    }
+    __syncthreads();
+    float I[16];
+    big_fft<6>(tb, sm, 1, r * K::PADM, A.tw,                         // pass B: column m = r
+        [&](int i) { return i < n ? Tm[i * TP + r] : make_float2(0.0f, 0.0f); },
+        [&](int, const float2 x, int slot) { I[slot] = fmaf(x.x, x.x, x.y * x.y); });
+    __syncthreads();                                                 // every thread has finished reading Tm
+    {
+        constexpr int RL = K::R1, NSL = 16, Q = 16 / RL;            // index arithmetic of the last pass (two passes)
+#pragma unroll
+        for (int qq = 0; qq < Q; ++qq) {
+            const int bb = tb + qq * T;
+            const int o0 = (bb / NSL) * (NSL * RL) + (bb & (NSL - 1));
+#pragma unroll
+            for (int kk = 0; kk < RL; ++kk) Ib[(o0 + kk * NSL) * TP + r] = I[qq * RL + kk];     // Ib[row k][column m]
+        }
+    }
+    __syncthreads();
+    // binning: pixel (pr, pc) sums rows k0 + pr beta .. and columns k0 + pc beta ..; 4 threads per pixel
+    const int beta = A.beta, part = tid & 3;
+    for (int px = tid >> 2; px < P * P; px += 64) {
+        const int pr = px / P, pc = px - pr * P;
+        float s = 0.0f;
+        for (int e = part; e < beta * beta; e += 4) {
+            const int er = e / beta, ec = e - er * beta;
+            s += Ib[(A.k0 + pr * beta + er) * TP + A.k0 + pc * beta + ec];
+        }
+        s += __shfl_xor_sync(0xffffffffu, s, 1);
+        s += __shfl_xor_sync(0xffffffffu, s, 2);
+        if (part == 0) out[px] = s * A.norm;
+    }
+}
+
 // ---- host side -------------------------------------------------------------------------------
 size_t sh_big_scratch_bytes(const ao_geometry*, const WfsH& w)
 {
+    if (w.M == 64) return 0;                                  // k_sh_mid64 keeps the whole transform in shared memory
     return sizeof(float2) * (size_t)w.grp.src.size() * w.n_sub * w.n_sub * w.n * w.M;
 }
 
@@ -331,10 +418,31 @@ cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, boo
                           long long step_stride, int n_steps, float2* scratch, size_t scratch_bytes, float* images,
                           cudaStream_t st)
 {
-    if (!sh_big_fast(w)) return launch_sh_big_generic(g, w, phase, api_layout, step_stride, n_steps, scratch, images, st);
     const int n_sel = (int)w.grp.src.size(), nsa = w.n_sub * w.n_sub;
     if (n_sel == 0 || n_steps <= 0) return cudaSuccess;
     cudaError_t e;
+    if (w.M == 64) {      // whole subaperture per CTA
+        const size_t smem = sizeof(float2) * (size_t)(64 * BigCfg<6>::PADM) +
+                            std::max(sizeof(float2) * (size_t)w.n * 65, sizeof(float) * (size_t)64 * 65);
+        if ((e = cudaFuncSetAttribute(k_sh_mid64, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        MidArgs m;
+        m.phase = phase; m.step_stride = step_stride; m.off = api_layout ? w.grp.d_off_api : w.grp.d_off_stage;
+        m.n_sel = n_sel; m.amp = w.d_amp; m.valid = w.d_valid; m.n_sub = w.n_sub; m.n = w.n;
+        m.tw = w.d_twf; m.pre = w.d_pre; m.beta = w.beta; m.P = w.P; m.k0 = (w.M - w.beta * w.P) / 2;
+        m.norm = (float)(1.0 / ((double)w.M * w.M * (double)w.n * w.n));
+        const long long total = (long long)n_steps * n_sel * nsa;
+        const long long chunk = 0x7fffffffLL / ((long long)n_sel * nsa) * ((long long)n_sel * nsa);
+        for (long long b0 = 0; b0 < total; b0 += chunk) {
+            const long long nb = total - b0 < chunk ? total - b0 : chunk;
+            m.phase = phase + (size_t)(b0 / ((long long)n_sel * nsa)) * step_stride;
+            m.out = images + (size_t)b0 * w.P * w.P;
+            k_sh_mid64<<<(unsigned)nb, 256, smem, st>>>(m);
+            g->launches++;
+            if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        }
+        return cudaSuccess;
+    }
+    if (!sh_big_fast(w)) return launch_sh_big_generic(g, w, phase, api_layout, step_stride, n_steps, scratch, images, st);
     const unsigned batch = (unsigned)(n_sel * nsa);
     // as many steps per launch pair as the scratch holds (at most 4: the intermediate should stay inside L2)
     const size_t per_step = sh_big_scratch_bytes(g, w);
