@@ -63,7 +63,7 @@ struct TiledTrace2Args {
     float* phase;
 };
 
-template <bool ANYDU>
+template <int MODE>
 __global__ void __launch_bounds__(kFusedThreads, 4)
 k_trace_tiled2(const TiledTrace2Args A)
 {
@@ -80,7 +80,7 @@ k_trace_tiled2(const TiledTrace2Args A)
     if (jfirst >= sp.N || ifirst >= sp.N) return;          // CTA-uniform
     u64 acc[kKS * kTR];
     double refsum[2];
-    trace2_tile<kFusedThreads, true, ANYDU>(A.T, sp, S, smem, jfirst, ifirst, A.T.step0 + 2 * kp, acc, refsum);
+    trace2_tile<kFusedThreads, true, MODE>(A.T, sp, S, smem, jfirst, ifirst, A.T.step0 + 2 * kp, acc, refsum);
     const int j0 = jfirst + tid, j1 = j0 + kFusedThreads;
 #pragma unroll
     for (int s = 0; s < kKS; ++s) {
@@ -155,7 +155,7 @@ cudaError_t launch_trace_tiled(ao_geometry* g, const Group& grp, bool api_layout
     if (n_sel == 0 || n_steps <= 0) return cudaSuccess;
     const Tile2Plan p2 = plan_tiles2(g, grp.src, dt, 0);
     if (p2.ok && !getenv("AO_TRACE_OLD")) {
-        auto kern2 = p2.anydu ? k_trace_tiled2<true> : k_trace_tiled2<false>;
+        auto kern2 = !p2.anydu ? k_trace_tiled2<0> : (p2.quad ? k_trace_tiled2<2> : k_trace_tiled2<1>);
         cudaError_t e2 = cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p2.smem);
         if (e2 != cudaSuccess) return e2;
         TiledTrace2Args a;

@@ -58,7 +58,7 @@ struct __align__(16) Trace2Shared {
 
 __host__ __device__ inline size_t trace2_sched_bytes(int n_layers)
 {
-    return (size_t)n_layers * sizeof(LayerT) + (sizeof(float4) * kTR + sizeof(int) * 4) * kKS * kT2MaxStages;
+    return (size_t)n_layers * sizeof(LayerT) + (sizeof(float4) * kTR + sizeof(int) * 8) * kKS * kT2MaxStages;
 }
 
 // ---- the 16 output rows of one (layer, step): straight-line row march ----
@@ -114,6 +114,30 @@ __device__ __forceinline__ void t2_march_any(u64 (&acc)[kKS * kTR], const uint32
     }
 }
 
+// For du <= 2/3 (fine WFS grids: c4 at M = 64 has du ~ 0.3): four consecutive output rows lie within three
+// screen-row intervals, so a group of four rows builds four x-interpolated rows X[r_g .. r_g + 3] once (4 tap loads
+// per output row, as in t2_march) and every row is a four-weight combination of them (two weights non-zero).
+// Table entry of row i: its four weights; gtab: the byte offsets of the four groups' first row relative to X[r_0].
+template <int OFF>
+__device__ __forceinline__ void t2_march_quad(u64 (&acc)[kKS * kTR], const uint32_t tp0, const uint32_t tp1, const uint32_t pb,
+                                              const u64 fx, const u64 ref, const uint32_t wtab, const uint32_t gtab)
+{
+    const float4 go = lds_f32x4(gtab);
+    const uint32_t goff[4] = {__float_as_uint(go.x), __float_as_uint(go.y), __float_as_uint(go.z), __float_as_uint(go.w)};
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+        const uint32_t a0 = tp0 + goff[g], a1 = tp1 + goff[g];
+        const u64 x0 = t2_xrow(a0, a1, fx, ref), x1 = t2_xrow(a0 + pb, a1 + pb, fx, ref);
+        const u64 x2 = t2_xrow(a0 + 2 * pb, a1 + 2 * pb, fx, ref), x3 = t2_xrow(a0 + 3 * pb, a1 + 3 * pb, fx, ref);
+#pragma unroll
+        for (int i = 4 * g; i < 4 * g + 4; ++i) {
+            const float4 w = lds_f32x4(wtab + 16u * (uint32_t)i);
+            acc[OFF + i] = fma2(pack2(w.w, w.w), x3, fma2(pack2(w.z, w.z), x2, fma2(pack2(w.y, w.y), x1,
+                           fma2(pack2(w.x, w.x), x0, acc[OFF + i]))));
+        }
+    }
+}
+
 // Ray-trace one tile for two steps: rows ifirst .. ifirst+15, columns jfirst + {tid, tid + NT} of source `sp` at
 // time steps step_first and step_first + 1.  acc[s * 16 + i] receives the packed (column tid, column tid + NT)
 // layer sums of step s, row i, minus warp-uniform piston references (the same for both steps); with REFSUM
@@ -121,7 +145,7 @@ __device__ __forceinline__ void t2_march_any(u64 (&acc)[kKS * kTR], const uint32
 // `dyn`: dynamic shared memory, 128-byte aligned: [ns][rows][pitch] floats, then trace2_sched_bytes(n_layers).
 // All NT threads call it.  On return every thread has finished reading the stages, but other warps may not
 // have: __syncthreads() before reusing the memory.
-template <int NT, bool REFSUM, bool ANYDU>
+template <int NT, bool REFSUM, int MODE>
 __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& sp, Trace2Shared& S, unsigned char* dyn,
                                             const int jfirst, const int ifirst, const long long step_first,
                                             u64 (&acc)[kKS * kTR], double (&refsum)[2])
@@ -134,6 +158,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
     LayerT* L = reinterpret_cast<LayerT*>(dyn + (size_t)ns * tile_floats * sizeof(float));
     float4* Wt = reinterpret_cast<float4*>(L + A.n_layers);       // [stage][step][row] table entries
     int* R0 = reinterpret_cast<int*>(Wt + kT2MaxStages * kKS * kTR);   // [stage][step] box row of the top tap of row 0
+    int* G = R0 + 4 * kKS * kT2MaxStages;                              // [stage][step][4] group offsets of the quad march
 
     if (tid == 0) {
         int na = 0;
@@ -167,7 +192,8 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             const long long c_lo = (long long)floor(uf[s]) & ~3LL;                         // 16-byte aligned start
             const long long c_hi = (long long)floor(fma((double)(NCOL - 1), du, uf[s])) + 2;
             const long long r_lo = (long long)floor(vf[s]);
-            const long long r_hi = (long long)floor(fma((double)(kTR - 1), du, vf[s])) + 1;
+            long long r_hi = (long long)floor(fma((double)(kTR - 1), du, vf[s])) + 1;
+            if (MODE == 2) r_hi = max(r_hi, (long long)floor(fma((double)(kTR - 4), du, vf[s])) + 3);   // last group's fourth row
             if (s == 0 || c_lo < cmin) cmin = c_lo;
             if (s == 0 || c_hi > cmax) cmax = c_hi;
             if (s == 0 || r_lo < rmin) rmin = r_lo;
@@ -210,7 +236,17 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             }
             const double fy = v - (double)r;
             const float w0 = (float)(1.0 - fy);
-            if (ANYDU) {
+            if (MODE == 2) {
+                // rows in groups of four share four x-interpolated screen rows starting at the group's first top row
+                const long long ru = (long long)floor(v);
+                const long long rg = __shfl_sync(0xffffffffu, ru, lane & ~3);
+                const double fu = v - (double)ru;
+                const int j = (int)(ru - rg);                                    // 0 .. 2 for du <= 2/3
+                const float c0 = (float)(1.0 - fu), c1 = (float)fu;
+                Wt[stage * (kKS * kTR) + lane] = make_float4(j == 0 ? c0 : 0.0f, j == 0 ? c1 : (j == 1 ? c0 : 0.0f),
+                                                              j == 1 ? c1 : (j == 2 ? c0 : 0.0f), j == 2 ? c1 : 0.0f);
+                if ((i & 3) == 0) G[(stage * kKS + s) * 4 + (i >> 2)] = (int)(ru - r0) * pitch * 4;
+            } else if (MODE == 1) {
                 const long long ru = (long long)floor(v);                       // unclamped: rows may advance by 2 or more
                 const double fu = v - (double)ru;
                 Wt[stage * (kKS * kTR) + lane] = make_float4((float)(1.0 - fu), (float)fu,
@@ -282,7 +318,8 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
                 const uint32_t rowb = tile_s + (uint32_t)ro0 * pb;
                 const uint32_t t0 = rowb + (uint32_t)(U0 >> 32) * 4u, t1 = rowb + (uint32_t)(U1 >> 32) * 4u;
                 const uint32_t wt_s = w_s + (uint32_t)(stage * kKS + 0) * (kTR * 16);
-                if (ANYDU) t2_march_any<0>(acc, t0, t1, pb, fx, ref, wt_s);
+                if (MODE == 2) t2_march_quad<0>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 0) * 4));
+                else if (MODE == 1) t2_march_any<0>(acc, t0, t1, pb, fx, ref, wt_s);
                 else t2_march<0>(acc, t0, t1, fx, ref, wt_s);
             }
             {
@@ -291,7 +328,8 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
                 const uint32_t rowb = tile_s + (uint32_t)ro1 * pb;
                 const uint32_t t0 = rowb + (uint32_t)(U0 >> 32) * 4u, t1 = rowb + (uint32_t)(U1 >> 32) * 4u;
                 const uint32_t wt_s = w_s + (uint32_t)(stage * kKS + 1) * (kTR * 16);
-                if (ANYDU) t2_march_any<kTR>(acc, t0, t1, pb, fx, ref, wt_s);
+                if (MODE == 2) t2_march_quad<kTR>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 1) * 4));
+                else if (MODE == 1) t2_march_any<kTR>(acc, t0, t1, pb, fx, ref, wt_s);
                 else t2_march<kTR>(acc, t0, t1, fx, ref, wt_s);
             }
         }
