@@ -353,3 +353,17 @@ def test_forward_matches_separate_calls():
     for a, b in zip(got_s, ref_s):
         assert torch.equal(a, b)
     assert torch.allclose(got_p, 2.0 * ref_p, rtol=1e-6, atol=0.0)
+
+
+def test_fft64_sensor_with_cropped_detector_window():
+    """M = 64 sensors run one CTA per subaperture (both FFT passes in shared memory).  A detector that keeps the
+    central 48 of 64 FFT pixels in 4 x 4 bins (k0 = 8, P = 12) exercises the window and binning arithmetic away from
+    the c4 default (8 x 8 bins of the whole field); fine LGS grid: the phase comes from the quad row march."""
+    cfg = inputs.make_config(4, n_sub=6, screen_n=1024, n_steps=3, lgs_fft=64)
+    cfg.wfs[0].bin, cfg.wfs[0].n_pix = 4, 12
+    ref = oracle.forward(cfg, 2, 3)
+    geo = _geo(cfg, 3)
+    import torch
+    img, slp = geo.sh_images(0, None, 2, 3, cfg.dt_s)
+    torch.cuda.synchronize()
+    check_wfs(cfg, geo, ref, 0, img, slp, 3, cfg.name)
