@@ -517,15 +517,18 @@ static int forward_chunk(ao_geometry* g, int64_t step0, int n_steps, double dt_s
         AO_CUDA(cudaEventRecord(g->ev_fork, st), "fork record");
         AO_CUDA(cudaStreamWaitEvent(g->side, g->ev_fork, 0), "fork wait");
     }
-    for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
-        const WfsH& w = g->wfs[wi];
-        if (!slopes || !slopes[wi] || w.grp.src.empty()) continue;
-        rc = run_wfs(g, (int)wi, nullptr, step0, n_steps, dt_s, noise, nullptr, slopes[wi], on_side[wi] ? sw : st);
-        if (rc) return rc;
-    }
-    if (want_psf) {
-        rc = run_psf(g, nullptr, step0, n_steps, dt_s, psf, accumulate, sw);
-        if (rc) return rc;
+    // the short kernels are submitted first so that they start at once; the long fused launch fills in behind them
+    for (int pass = 0; pass < 2; ++pass) {
+        for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
+            const WfsH& w = g->wfs[wi];
+            if (!slopes || !slopes[wi] || w.grp.src.empty() || (on_side[wi] != 0) != (pass == 0)) continue;
+            rc = run_wfs(g, (int)wi, nullptr, step0, n_steps, dt_s, noise, nullptr, slopes[wi], on_side[wi] ? sw : st);
+            if (rc) return rc;
+        }
+        if (pass == 0 && want_psf) {
+            rc = run_psf(g, nullptr, step0, n_steps, dt_s, psf, accumulate, sw);
+            if (rc) return rc;
+        }
     }
     if (fork) {
         AO_CUDA(cudaEventRecord(g->ev_join, g->side), "join record");
