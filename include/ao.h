@@ -171,6 +171,16 @@ int ao_centroids(ao_geometry* g, int wfs_index, const float* images_dev, int n_i
 int ao_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, double dt_s,
            float* psf_dev, int accumulate, void* cuda_stream);
 
+/* ao_set_phase_map -- static additive phase map of one source (section 2.3: telescope aberration
+ * maps such as M1 scalloping and the NGS-WFS mis-positioning tip/tilt are "summed to the open loop WF"):
+ *   phi_s[k, i, j] <- phi_s[k, i, j] + map[i][j]  for every time step k,
+ * applied wherever the library produces phi_s (ao_trace_layers and every phase_dev == NULL path: ao_sh_images,
+ * ao_psf, ao_forward, ao_forward_host).  map_dev: [N_s][N_s] fp32 radians AT THE SOURCE'S WAVELENGTH on the source's
+ * grid (ao_trace_layers layout of one source), DEVICE pointer, borrowed until replaced, cleared with NULL, or the
+ * handle is destroyed.  Synchronises the device (the call updates a table that launches in flight may be reading).
+ * Errors: AO_ERR_INVALID_ARG for a bad handle or source index. */
+int ao_set_phase_map(ao_geometry* g, int source, const float* map_dev);
+
 /* ao_forward -- the whole step with DEVICE buffers: ray-trace + every WFS (slopes only, noiseless unless
  * `noise`) + every science PSF for n_steps steps (the per-time-step forward model).
  * Same results as one ao_sh_images(phase_dev = NULL, images_dev = NULL) per WFS plus ao_psf(phase_dev = NULL),

@@ -183,7 +183,9 @@ def forward(cfg, step0: int = 0, n_steps: int = 1, *, want_phase=True, want_wfs=
       slopes[s]  : [n_steps][2][n_sub^2]      (from noisy images if noise_on else noiseless)
       valid[w]   : [n_sub^2] uint8 per WFS
       psf[s]     : [M][M] long-exposure SUM over the steps (science sources)
-    Plain loop over steps and sources; every number comes from ao_oracle.c.
+    cfg.phase_maps[s] (optional, [N_s][N_s] radians at the source's wavelength) is added to the traced phase of
+    source s at every step (section 2.3) before the WFS and the PSF see it.
+    Plain loop over steps and sources; every number comes from ao_oracle.c (the map sum is one numpy add).
     """
     res = {"phase": {}, "images": {}, "noisy": {}, "counts": {}, "slopes": {}, "valid": {}, "psf": {}}
     srcs = range(len(cfg.sources)) if sources is None else sources
@@ -202,6 +204,9 @@ def forward(cfg, step0: int = 0, n_steps: int = 1, *, want_phase=True, want_wfs=
             t = (step0 + k) * cfg.dt_s
             ph = trace(cfg.layers, src.theta_x_rad, src.theta_y_rad, src.altitude_m, src.lambda_m,
                        cfg.lambda_ref_m, N, d, t)
+            pm = getattr(cfg, "phase_maps", {}).get(s)
+            if pm is not None:      # static aberration map summed to the open-loop wavefront (section 2.3)
+                ph = ph + np.asarray(pm, dtype=np.float64)
             if want_phase:
                 ph_list.append(ph)
             if w >= 0 and want_wfs:

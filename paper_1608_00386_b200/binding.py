@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "AO_OK", 1: "AO_ERR_INVALID_ARG", 2: "AO_ERR_SHAPE", 3: "AO_E
 # every symbol include/ao.h declares
 EXPORTS = ["ao_geometry_create", "ao_geometry_destroy", "ao_workspace_bytes", "ao_set_workspace",
            "ao_phase_elems_per_step", "ao_phase_offset", "ao_wfs_valid", "ao_trace_layers",
-           "ao_sh_images", "ao_centroids", "ao_psf", "ao_forward", "ao_forward_host", "ao_launch_count",
+           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_phase_map", "ao_forward", "ao_forward_host", "ao_launch_count",
            "ao_last_error", "ao_version"]
 
 
@@ -82,6 +82,7 @@ def load_library():
     L.ao_sh_images.argtypes = [vp, i32, vp, i64, i32, dbl, C.POINTER(ao_noise), vp, vp, vp]
     L.ao_centroids.argtypes = [vp, i32, vp, i32, vp, vp]
     L.ao_psf.argtypes = [vp, vp, i64, i32, dbl, vp, i32, vp]
+    L.ao_set_phase_map.argtypes = [vp, i32, vp]
     L.ao_forward.argtypes = [vp, i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, i32, vp]
     L.ao_forward_host.argtypes = [vp, C.POINTER(vp), i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, vp]
     L.ao_launch_count.argtypes = [vp]; L.ao_launch_count.restype = i64
@@ -152,7 +153,10 @@ class Geometry:
                                            len(cfg.sources), cfg.lambda_ref_m, cfg.psf_fft, C.byref(h)))
         self.handle = h
         self.workspace = None
+        self.phase_maps = {}
         self.set_workspace_steps(workspace_steps)
+        for si, m in getattr(cfg, "phase_maps", {}).items():
+            self.set_phase_map(si, m)
 
     # ---- lifetime ----
     def close(self):
@@ -165,6 +169,18 @@ class Geometry:
             self.close()
         except Exception:
             pass
+
+    def set_phase_map(self, source: int, phase_map):
+        """ao_set_phase_map: additive [N_s][N_s] phase map (numpy array, CUDA tensor, or None to clear)."""
+        import torch
+        if phase_map is None:
+            self.phase_maps.pop(source, None)
+            _check(self.lib.ao_set_phase_map(self.handle, int(source), None))
+            return
+        t = torch.as_tensor(np.ascontiguousarray(phase_map, dtype=np.float32) if isinstance(phase_map, np.ndarray)
+                            else phase_map, dtype=torch.float32).to(self.device).contiguous()
+        self.phase_maps[source] = t                      # borrowed by the library: keep it alive
+        _check(self.lib.ao_set_phase_map(self.handle, int(source), _ptr(t)))
 
     # ---- sizes ----
     def workspace_bytes(self, max_steps: int) -> int:

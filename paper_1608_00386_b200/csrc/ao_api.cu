@@ -376,6 +376,7 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
         sp.H = src[i].altitude_m; sp.inv_H = std::isinf(sp.H) ? 0.0 : 1.0 / sp.H;
         sp.scale = lambda_ref_m / src[i].lambda_m;
         sp.phase_off = off;
+        sp.map = nullptr;
         off += (long long)sp.N * sp.N;
         g->all.src.push_back(i);
         if (sp.wfs < 0) g->sci.src.push_back(i); else g->wfs[sp.wfs].grp.src.push_back(i);
@@ -534,6 +535,16 @@ static int forward_chunk(ao_geometry* g, int64_t step0, int n_steps, double dt_s
         AO_CUDA(cudaEventRecord(g->ev_join, g->side), "join record");
         AO_CUDA(cudaStreamWaitEvent(st, g->ev_join, 0), "join wait");
     }
+    return AO_OK;
+}
+
+int ao_set_phase_map(ao_geometry* g, int source, const float* map_dev)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (source < 0 || source >= (int)g->sources.size()) return fail(AO_ERR_INVALID_ARG, "ao_set_phase_map: bad source index");
+    AO_CUDA(cudaDeviceSynchronize(), "synchronize before the source table update");
+    g->sources[source].map = map_dev;
+    AO_CUDA(cudaMemcpy(g->d_sources + source, &g->sources[source], sizeof(SourceP), cudaMemcpyHostToDevice), "source table update");
     return AO_OK;
 }
 

@@ -31,6 +31,7 @@ struct SourceP {
     double inv_H;          // 1/H (0 for inf)
     double scale;          // lambda_ref / lambda_s
     long long phase_off;   // element offset inside one step of the caller's phase buffer
+    const float* map;      // additive phase map [N][N], radians at the source's wavelength, or NULL (ao_set_phase_map)
 };
 
 // A group of sources processed together (all / those of one WFS / science directions).

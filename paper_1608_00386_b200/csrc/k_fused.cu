@@ -82,7 +82,7 @@ struct FusedCfg {
     static_assert(kTR % n == 0 && NT % n == 0 && n <= 32, "bad fused configuration");
 };
 
-template <int M, bool NOISE, bool ANYDU>
+template <int M, bool NOISE, bool ANYDU, bool MAPS>
 __global__ void __launch_bounds__(kFusedThreads, 4)
 k_fused(const FusedArgs A)
 {
@@ -110,6 +110,7 @@ k_fused(const FusedArgs A)
     // ---- phase B: image formation, one (subaperture row, column slot) round at a time ----
     float2* xch = reinterpret_cast<float2*>(smem);
     const float scale = (float)sp.scale;
+    const float* mp = MAPS ? sp.map : nullptr;             // additive phase map of this source or NULL (ao_set_phase_map)
     const int g = tid / n, b = tid - g * n;                // subaperture in round, column in subaperture
     float2* xs = xch + (size_t)g * K::SUB_STRIDE;
 #pragma unroll 1
@@ -134,7 +135,8 @@ k_fused(const FusedArgs A)
 #pragma unroll
                 for (int hh = 1; hh < K::HS; ++hh) v = (hs == hh) ? acc[hh * n + i] : v;
                 const float2 f = unpack2(v);
-                const float ph = (c ? f.y : f.x) * scale;
+                float ph = (c ? f.y : f.x) * scale;
+                if (MAPS && mp && active) ph += __ldg(mp + (size_t)(p * n + i) * N + (size_t)q * n + b);
                 const float Am = active ? __ldg(ap + (size_t)i * N) : 0.0f;
                 float s, co;
                 sincos_reduced(ph, &s, &co);
@@ -239,8 +241,13 @@ template <int M>
 static cudaError_t launch_fused_variant(ao_geometry* g, const WfsH& w, FusedArgs a, const Tile2Plan& pl, int n_steps,
                                         cudaStream_t st)
 {
-    auto kern = pl.anydu ? (a.nz.on ? k_fused<M, true, true> : k_fused<M, false, true>)
-                         : (a.nz.on ? k_fused<M, true, false> : k_fused<M, false, false>);
+    bool maps = false;                                     // the map-free kernel keeps its register budget
+    for (int si : w.grp.src) maps = maps || g->sources[si].map != nullptr;
+    void (*kern)(const FusedArgs);
+    if (maps) kern = pl.anydu ? (a.nz.on ? k_fused<M, true, true, true> : k_fused<M, false, true, true>)
+                              : (a.nz.on ? k_fused<M, true, false, true> : k_fused<M, false, false, true>);
+    else kern = pl.anydu ? (a.nz.on ? k_fused<M, true, true, false> : k_fused<M, false, true, false>)
+                         : (a.nz.on ? k_fused<M, true, false, false> : k_fused<M, false, false, false>);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     const size_t nsa = (size_t)w.n_sub * w.n_sub;

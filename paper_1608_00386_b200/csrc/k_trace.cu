@@ -67,7 +67,8 @@ k_trace(const LayerP* __restrict__ layers, int n_layers, const SourceP* __restri
         const float bot = fmaf(fx, s11 - s10, s10);
         acc += (double)fmaf(fy, bot - top, top);
     }
-    phase[(size_t)k * step_stride + off[si] + (size_t)i * sp.N + j] = (float)(acc * sp.scale);
+    const size_t o = (size_t)i * sp.N + j;
+    phase[(size_t)k * step_stride + off[si] + o] = (float)(acc * sp.scale + (sp.map ? (double)sp.map[o] : 0.0));
 }
 
 cudaError_t launch_trace(ao_geometry* g, const Group& grp, bool api_layout, long long step_stride,

@@ -54,8 +54,9 @@ k_trace_tiled2(const TiledTrace2Args A)
             const int row = ifirst + i;
             if (row < sp.N) {
                 const float2 f = unpack2(acc[s * kTR + i]);
-                if (j0 < sp.N) out[(size_t)row * sp.N + j0] = (float)(((double)f.x + refsum[0]) * sp.scale);
-                if (j1 < sp.N) out[(size_t)row * sp.N + j1] = (float)(((double)f.y + refsum[1]) * sp.scale);
+                const size_t o0 = (size_t)row * sp.N + j0, o1 = (size_t)row * sp.N + j1;
+                if (j0 < sp.N) out[o0] = (float)(((double)f.x + refsum[0]) * sp.scale + (sp.map ? (double)sp.map[o0] : 0.0));
+                if (j1 < sp.N) out[o1] = (float)(((double)f.y + refsum[1]) * sp.scale + (sp.map ? (double)sp.map[o1] : 0.0));
             }
         }
     }

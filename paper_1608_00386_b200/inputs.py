@@ -94,6 +94,8 @@ class Config:
     r0_m: float = R0_REF
     L0_m: float = L0_REF
     notes: dict = field(default_factory=dict)
+    # static additive phase maps: source index -> [N_s][N_s] float32 radians at the source's wavelength
+    phase_maps: dict = field(default_factory=dict)
 
     # ---- derived shapes (no arithmetic of the method; only sizes) ----
     def grid_n(self, s: int) -> int:

@@ -367,3 +367,50 @@ def test_fft64_sensor_with_cropped_detector_window():
     img, slp = geo.sh_images(0, None, 2, 3, cfg.dt_s)
     torch.cuda.synchronize()
     check_wfs(cfg, geo, ref, 0, img, slp, 3, cfg.name)
+
+
+def _smooth_map(rng, N, rms):
+    """Low-order random map (a few rad): bilinear upsampling of an 6 x 6 normal grid; harness data only."""
+    g = rng.normal(size=(6, 6))
+    x = np.linspace(0, 5, N)
+    i0 = np.minimum(x.astype(int), 4); f = x - i0
+    rows = g[i0] * (1 - f)[:, None] + g[i0 + 1] * f[:, None]
+    m = rows[:, i0] * (1 - f)[None, :] + rows[:, i0 + 1] * f[None, :]
+    return (rms * m).astype(np.float32)
+
+
+def test_phase_maps_all_paths():
+    """ao_set_phase_map (aberration maps summed to the open-loop wavefront): every phase producer
+    -- tiled writer, fused kernel, big-FFT staging, PSF staging -- against the oracle; then clearing one map."""
+    import torch
+    cfg = inputs.make_config(3, n_sub=8, screen_n=512, n_steps=2)
+    rng = np.random.default_rng(11)
+    cfg.phase_maps = {s: _smooth_map(rng, cfg.grid_n(s), 2.0) for s in (0, 3, 6, 7, 9, 12)}   # LGS, NGS, science
+    out, ref = _check_all(cfg, 2, step0=3)
+    geo = out["geo"]
+    # clear the map of LGS source 0: its slopes must go back to the map-free oracle values
+    geo.set_phase_map(0, None)
+    del cfg.phase_maps[0]
+    ref0 = oracle.forward(cfg, 3, 2, sources=[0])
+    img, slp = geo.sh_images(0, None, 3, 2, cfg.dt_s)
+    torch.cuda.synchronize()
+    d = np.abs(slp[:, 0].cpu().numpy() - ref0["slopes"][0]).max()
+    assert d <= SLOPE_TOL, d
+
+
+def test_phase_map_per_sample_trace_path_and_errors():
+    """The per-sample kernel (screens whose side is not a multiple of 4 are outside the tile plan) adds the map too;
+    bad source indices are rejected."""
+    from paper_1608_00386_b200 import binding
+    cfg = inputs.make_config(0)
+    S = 254                                               # not a multiple of 4: k_trace path
+    cfg.layers[0].screen = np.ascontiguousarray(cfg.layers[0].screen[:S, :S]); cfg.layers[0].n = S
+    cfg.phase_maps = {0: _smooth_map(np.random.default_rng(2), cfg.grid_n(0), 1.0)}
+    ref = oracle.forward(cfg, 0, 1)
+    geo = _geo(cfg, 1)
+    phase = geo.trace_layers(0, 1, cfg.dt_s)
+    import torch
+    torch.cuda.synchronize()
+    _check_phase(cfg, geo, phase, ref, 1)
+    with pytest.raises(binding.AoError):
+        geo.set_phase_map(5, cfg.phase_maps[0])

@@ -561,3 +561,39 @@ def test_configs_have_survey_shapes():
     assert abs(sum(l.weight for l in c4.layers) - 1.0) < 1e-12 and len(c4.sources) == 10
     c1 = inputs.make_config(1, with_screens=False)
     assert c1.wfs[0].fft == 24 and c1.pupil.r_in_m == 5.5 and c1.pupil.r_out_m == 19.2
+
+
+# ----------------------------------------------------------------------------- phase maps
+@pytest.mark.parametrize("entry", [e for e in GOLD["cog"] if e[0] == (8, 16, 2, 8)])
+def test_phase_map_tilt_on_flat_atmosphere_gives_golden_cog(entry):
+    """A static map alpha * j summed to the (flat) open-loop wavefront is a pure x-tilt of alpha rad/sample: every
+    fully lit subaperture of c0 must show the closed-form CoG of SURVEY.md section 8(c), and no y-slope."""
+    (n, M, beta, P), t, cog = entry
+    cfg = inputs.make_config(0)
+    cfg.layers[0].screen = np.zeros_like(cfg.layers[0].screen)
+    N = cfg.wfs[0].n_sub * n
+    alpha = 2.0 * np.pi * t / M
+    cfg.phase_maps = {0: np.tile((alpha * np.arange(N)).astype(np.float64), (N, 1))}
+    res = oracle.forward(cfg, 0, 1)
+    assert np.allclose(res["phase"][0][0], cfg.phase_maps[0], atol=0.0)
+    amp = cfg.wfs[0].amp.reshape(cfg.wfs[0].n_sub, n, cfg.wfs[0].n_sub, n)
+    full = (amp.min(axis=(1, 3)) == 1.0).ravel()
+    assert full.sum() == 60                                   # SURVEY.md section 8(c) O1: 60 fully lit subapertures
+    sx, sy = res["slopes"][0][0]
+    assert np.abs(sx[full] - cog).max() < 1e-10 and np.abs(sy[full]).max() < 1e-10
+
+
+def test_phase_map_adds_to_phase_and_piston_map_changes_nothing_else():
+    cfg = inputs.make_config(0)
+    base = oracle.forward(cfg, 3, 1)
+    rng = np.random.default_rng(5)
+    N = cfg.grid_n(0)
+    m = rng.normal(size=(N, N)).astype(np.float32)
+    cfg.phase_maps = {0: m}
+    with_map = oracle.forward(cfg, 3, 1)
+    assert np.array_equal(with_map["phase"][0][0], base["phase"][0][0] + m.astype(np.float64))
+    assert np.abs(with_map["slopes"][0] - base["slopes"][0]).max() > 1e-3          # a random map does move the spots
+    cfg.phase_maps = {0: np.full((N, N), 1.2345, np.float32)}                       # piston: invisible to |FFT|^2
+    piston = oracle.forward(cfg, 3, 1)
+    assert np.abs(piston["images"][0] - base["images"][0]).max() < 1e-12
+    assert np.abs(piston["slopes"][0] - base["slopes"][0]).max() < 1e-10
