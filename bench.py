@@ -190,6 +190,13 @@ def run_gpu(args):
     cfg = inputs.make_config(4, lgs_fft=args.lgs_fft, screen_n=args.screen_n, n_layers=args.layers,
                              device=dev, keep_on_device=True)
     geo = binding.Geometry(cfg, device=dev, workspace_steps=batch)
+    if args.phase_maps:      # NEXT-1: a static aberration map on every source, synthetic smooth field
+        gen = torch.Generator(device=dev); gen.manual_seed(1608)
+        for si in range(len(cfg.sources)):
+            n_s = cfg.grid_n(si)
+            coarse = torch.randn((1, 1, 8, 8), generator=gen, device=dev)
+            geo.set_phase_map(si, torch.nn.functional.interpolate(coarse, size=(n_s, n_s), mode="bilinear",
+                                                                  align_corners=True)[0, 0].contiguous())
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t_setup
     lgs, ngs = cfg.wfs[0], cfg.wfs[1]
@@ -299,7 +306,7 @@ def run_gpu(args):
                 "config": {"workload": cfg.name, "lgs": f"{n_lgs} LGS x {lgs.n_sub}x{lgs.n_sub} subaps, n={lgs.n_samp}, FFT {lgs.fft}, {lgs.n_pix}x{lgs.n_pix} px",
                            "ngs": f"{n_ngs} NGS x 2x2 subaps, n={ngs.n_samp}, FFT {ngs.fft}",
                            "psf": f"{n_sci} science PSF, FFT {cfg.psf_fft}", "layers": len(cfg.layers),
-                           "screen_n": cfg.layers[0].n, "steps_per_call": batch,
+                           "screen_n": cfg.layers[0].n, "steps_per_call": batch, "phase_maps": bool(args.phase_maps),
                            "valid_subaperture_frames_per_step": frames_per_step,
                            "grid_slot_frames_per_step": n_lgs * lgs.n_sub ** 2 + n_ngs * ngs.n_sub ** 2,
                            "l2_policy": "inputs larger than L2: 9.4 GB of screens, ~211 MB touched per step",
@@ -327,6 +334,7 @@ def main():
     ap.add_argument("--layers", type=int, default=35)
     ap.add_argument("--batch", type=int, default=50, help="time steps per C-ABI call")
     ap.add_argument("--serial", action="store_true", help="one C-ABI call per leg on one stream instead of ao_forward")
+    ap.add_argument("--phase-maps", action="store_true", help="set a static additive phase map on every source (ao_set_phase_map)")
     ap.add_argument("--skip-e2e", action="store_true")
     ap.add_argument("--skip-cpu", action="store_true")
     args = ap.parse_args()
