@@ -181,6 +181,18 @@ int ao_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, d
  * Errors: AO_ERR_INVALID_ARG for a bad handle or source index. */
 int ao_set_phase_map(ao_geometry* g, int source, const float* map_dev);
 
+/* ao_modes_to_map -- residual-phase entry (section 2.7: "residual = open loop WF - DM shape", the
+ * WFS then measures the residual; section 2.5: the calibration pushes mirror modes through the WFS):
+ *   map[i] = sign * sum_{m < n_modes} coeffs[m] * modes[m][i],  i < n_elems   (fp32, modes summed in index order).
+ * With map_dev registered once through ao_set_phase_map and sign = -1 this is the deformable-mirror shape
+ * subtracted from the open-loop wavefront of that source; the mode arrays (mirror modes projected on the
+ * source's grid, radians at its wavelength) and the coefficients are the caller's: modal bases and control are
+ * outside this library.  All pointers are DEVICE pointers: modes_dev [n_modes][n_elems], coeffs_dev [n_modes],
+ * map_dev [n_elems] (overwritten).  Asynchronous on cuda_stream: calls that follow on the same stream see the
+ * new map.  n_modes = 0 zeroes the map.  Errors: AO_ERR_INVALID_ARG for NULL pointers or negative sizes. */
+int ao_modes_to_map(ao_geometry* g, const float* modes_dev, int n_modes, long long n_elems,
+                    const float* coeffs_dev, float sign, float* map_dev, void* cuda_stream);
+
 /* ao_forward -- the whole step with DEVICE buffers: ray-trace + every WFS (slopes only, noiseless unless
  * `noise`) + every science PSF for n_steps steps (the per-time-step forward model).
  * Same results as one ao_sh_images(phase_dev = NULL, images_dev = NULL) per WFS plus ao_psf(phase_dev = NULL),

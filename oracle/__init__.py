@@ -172,6 +172,14 @@ def noise(images: np.ndarray, valid, seed: int, source: int, step: int, photons:
 
 
 # ------------------------------------------------------------------------------- step driver
+def modes_to_map(modes: np.ndarray, coeffs: np.ndarray, sign: float) -> np.ndarray:
+    """Residual-phase entry (PAPER.md:82 section 2.7, :74 section 2.5): map = sign * sum_m coeffs[m] modes[m], FP64.
+    The plain definition: one numpy contraction over the mode index."""
+    m = np.asarray(modes, dtype=np.float64)
+    c = np.asarray(coeffs, dtype=np.float64)
+    return float(sign) * np.tensordot(c, m, axes=(0, 0))
+
+
 def forward(cfg, step0: int = 0, n_steps: int = 1, *, want_phase=True, want_wfs=True,
             want_psf=True, noise_on=False, sources=None):
     """Run the whole forward model of `cfg` (inputs.Config) for steps step0..step0+n_steps-1.

@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "AO_OK", 1: "AO_ERR_INVALID_ARG", 2: "AO_ERR_SHAPE", 3: "AO_E
 # every symbol include/ao.h declares
 EXPORTS = ["ao_geometry_create", "ao_geometry_destroy", "ao_workspace_bytes", "ao_set_workspace",
            "ao_phase_elems_per_step", "ao_phase_offset", "ao_wfs_valid", "ao_trace_layers",
-           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_phase_map", "ao_forward", "ao_forward_host", "ao_launch_count",
+           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_phase_map", "ao_modes_to_map", "ao_forward", "ao_forward_host", "ao_launch_count",
            "ao_last_error", "ao_version"]
 
 
@@ -83,6 +83,7 @@ def load_library():
     L.ao_centroids.argtypes = [vp, i32, vp, i32, vp, vp]
     L.ao_psf.argtypes = [vp, vp, i64, i32, dbl, vp, i32, vp]
     L.ao_set_phase_map.argtypes = [vp, i32, vp]
+    L.ao_modes_to_map.argtypes = [vp, vp, i32, i64, vp, C.c_float, vp, vp]
     L.ao_forward.argtypes = [vp, i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, i32, vp]
     L.ao_forward_host.argtypes = [vp, C.POINTER(vp), i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, vp]
     L.ao_launch_count.argtypes = [vp]; L.ao_launch_count.restype = i64
@@ -181,6 +182,16 @@ class Geometry:
                             else phase_map, dtype=torch.float32).to(self.device).contiguous()
         self.phase_maps[source] = t                      # borrowed by the library: keep it alive
         _check(self.lib.ao_set_phase_map(self.handle, int(source), _ptr(t)))
+
+    def modes_to_map(self, modes, coeffs, sign: float, out):
+        """ao_modes_to_map: out[i] = sign * sum_m coeffs[m] modes[m][i] (CUDA float32 tensors; out is overwritten)."""
+        n_modes = int(modes.shape[0]) if modes is not None else 0
+        if modes is not None:
+            modes, coeffs = modes.contiguous(), coeffs.contiguous()      # [n_modes][n_elems] row-major, as the ABI says
+        assert out.is_contiguous()
+        _check(self.lib.ao_modes_to_map(self.handle, _ptr(modes), n_modes, int(out.numel()), _ptr(coeffs),
+                                        float(sign), _ptr(out), _stream()))
+        return out
 
     # ---- sizes ----
     def workspace_bytes(self, max_steps: int) -> int:

@@ -548,6 +548,16 @@ int ao_set_phase_map(ao_geometry* g, int source, const float* map_dev)
     return AO_OK;
 }
 
+int ao_modes_to_map(ao_geometry* g, const float* modes_dev, int n_modes, long long n_elems,
+                    const float* coeffs_dev, float sign, float* map_dev, void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (n_modes < 0 || n_elems < 0) return fail(AO_ERR_INVALID_ARG, "ao_modes_to_map: negative size");
+    if (!map_dev || (n_modes > 0 && (!modes_dev || !coeffs_dev))) return fail(AO_ERR_INVALID_ARG, "ao_modes_to_map: NULL pointer");
+    AO_CUDA(launch_modes_to_map(g, modes_dev, n_modes, n_elems, coeffs_dev, sign, map_dev, (cudaStream_t)cuda_stream), "modes_to_map");
+    return AO_OK;
+}
+
 int ao_forward(ao_geometry* g, int64_t step0, int n_steps, double dt_s, const ao_noise* noise,
                float* const* slopes_dev, float* psf_dev, int accumulate, void* cuda_stream)
 {

@@ -110,6 +110,9 @@ cudaError_t launch_sh_small(ao_geometry* g, const WfsH& w, const float* phase, b
 cudaError_t launch_centroids(ao_geometry* g, const WfsH& w, const float* images, int n_sets,
                              float* slopes, cudaStream_t st);
 
+cudaError_t launch_modes_to_map(ao_geometry* g, const float* modes, int n_modes, long long n_elems, const float* coeffs,
+                                float sign, float* map, cudaStream_t st);
+
 cudaError_t launch_noise(ao_geometry* g, const WfsH& w, float* images, int64_t step0, int n_steps,
                          const NoiseP& noise, cudaStream_t st);
 

@@ -217,6 +217,29 @@ cudaError_t launch_centroids(ao_geometry* g, const WfsH& w, const float* images,
 }
 
 // ------------------------------------------------------------------------------------------
+// ao_modes_to_map: map[i] = sign * sum_m coeffs[m] modes[m][i] (PAPER.md:82 residual phase, :74 calibration pushes).
+// HBM-bound: every mode array is read once, coalesced; the coefficients are warp-uniform loads.
+__global__ void __launch_bounds__(256)
+k_modes_to_map(const float* __restrict__ modes, int n_modes, long long n_elems, const float* __restrict__ coeffs,
+               float sign, float* __restrict__ map)
+{
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n_elems) return;
+    float acc = 0.0f;
+    for (int m = 0; m < n_modes; ++m) acc = fmaf(__ldg(coeffs + m), modes[(size_t)m * n_elems + i], acc);
+    map[i] = sign * acc;
+}
+
+cudaError_t launch_modes_to_map(ao_geometry* g, const float* modes, int n_modes, long long n_elems, const float* coeffs,
+                                float sign, float* map, cudaStream_t st)
+{
+    if (n_elems <= 0) return cudaSuccess;
+    k_modes_to_map<<<(unsigned)((n_elems + 255) / 256), 256, 0, st>>>(modes, n_modes, n_elems, coeffs, sign, map);
+    g->launches++;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
 // Stand-alone detector noise, in place on [n_steps][n_sel][nsa][P][P] normalised images.
 __global__ void __launch_bounds__(256)
 k_noise(float* __restrict__ images, const uint8_t* __restrict__ valid, const int* __restrict__ sel,

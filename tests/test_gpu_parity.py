@@ -414,3 +414,33 @@ def test_phase_map_per_sample_trace_path_and_errors():
     _check_phase(cfg, geo, phase, ref, 1)
     with pytest.raises(binding.AoError):
         geo.set_phase_map(5, cfg.phase_maps[0])
+
+
+def test_modes_to_map_and_closed_loop_residual():
+    """ao_modes_to_map against the oracle contraction; then the residual-phase use: the map buffer is
+    registered once with ao_set_phase_map and rewritten on the stream: the sensor sees open loop - DM shape."""
+    import torch
+    cfg = inputs.make_config(2, n_sub=9, screen_n=512, n_steps=2)
+    geo = _geo(cfg, 2)
+    rng = np.random.default_rng(21)
+    N = cfg.grid_n(0)
+    modes = np.ascontiguousarray(np.stack([_smooth_map(rng, N, 1.0) for _ in range(37)]))
+    coeffs = rng.normal(size=37).astype(np.float32)
+    d_modes, d_coeffs = torch.tensor(modes, device="cuda"), torch.tensor(coeffs, device="cuda")
+    d_map = torch.full((N, N), float("nan"), dtype=torch.float32, device="cuda")
+    geo.modes_to_map(d_modes, d_coeffs, -1.0, d_map)
+    torch.cuda.synchronize()
+    want = oracle.modes_to_map(modes, coeffs, -1.0)
+    assert rel_l2(d_map.cpu().numpy(), want) <= 1e-6
+    geo.set_phase_map(2, d_map)                               # LGS source 2 looks through the "mirror"
+    for trial in range(2):                                    # new coefficients: same registered buffer, no re-registration
+        c = rng.normal(size=37).astype(np.float32)
+        geo.modes_to_map(d_modes, torch.tensor(c, device="cuda"), -1.0, d_map)
+        img, slp = geo.sh_images(0, None, 7, 2, cfg.dt_s)
+        torch.cuda.synchronize()
+        cfg.phase_maps = {2: oracle.modes_to_map(modes, c, -1.0)}
+        ref = oracle.forward(cfg, 7, 2, want_phase=False)
+        check_wfs(cfg, geo, ref, 0, img, slp, 2, cfg.name + " residual")
+    geo.modes_to_map(None, None, 1.0, d_map)                  # no modes: zero map
+    torch.cuda.synchronize()
+    assert float(d_map.abs().max()) == 0.0

@@ -597,3 +597,38 @@ def test_phase_map_adds_to_phase_and_piston_map_changes_nothing_else():
     piston = oracle.forward(cfg, 3, 1)
     assert np.abs(piston["images"][0] - base["images"][0]).max() < 1e-12
     assert np.abs(piston["slopes"][0] - base["slopes"][0]).max() < 1e-10
+
+
+# ----------------------------------------------------------------------------- residual-phase entry
+def test_modes_to_map_brute_force_one_hot_and_linearity():
+    rng = np.random.default_rng(8)
+    modes = rng.normal(size=(5, 7, 3))
+    c = rng.normal(size=5)
+    got = oracle.modes_to_map(modes, c, -1.0)
+    want = np.zeros((7, 3))
+    for m in range(5):                                     # brute force, the definition written out
+        for i in range(7):
+            for j in range(3):
+                want[i, j] -= c[m] * modes[m, i, j]
+    assert np.abs(got - want).max() < 1e-14
+    one_hot = np.zeros(5); one_hot[3] = 2.5
+    assert np.array_equal(oracle.modes_to_map(modes, one_hot, 1.0), 2.5 * modes[3])
+    c2 = rng.normal(size=5)
+    assert np.abs(oracle.modes_to_map(modes, c + c2, 1.0) - oracle.modes_to_map(modes, c, 1.0)
+                  - oracle.modes_to_map(modes, c2, 1.0)).max() < 1e-14
+
+
+def test_residual_of_a_tilt_mode_cancels_a_tilted_wavefront():
+    """Closed loop in one line: open-loop tilt from a linear screen, minus coefficient x tilt mode with
+    the matching coefficient, leaves a flat residual: zero slopes on every valid subaperture."""
+    cfg = inputs.make_config(0)
+    g_px = 0.125
+    cfg.layers[0].screen = inputs.linear_screen(cfg.layers[0].n, 0.0, 0.0, g_px)
+    N = cfg.grid_n(0)
+    alpha = g_px * cfg.grid_pitch(0) / cfg.layers[0].pitch_m * cfg.lambda_ref_m / cfg.sources[0].lambda_m
+    mode = np.tile(np.arange(N, dtype=np.float64), (N, 1))[None]          # unit x-ramp, radians per sample
+    open_loop = oracle.forward(cfg, 0, 1)
+    assert np.abs(open_loop["slopes"][0][0][0]).max() > 0.05
+    cfg.phase_maps = {0: oracle.modes_to_map(mode, np.array([alpha]), -1.0)}
+    closed = oracle.forward(cfg, 0, 1)
+    assert np.abs(closed["slopes"][0]).max() < 1e-9
