@@ -272,6 +272,23 @@ def run_gpu(args):
                 "lgs_grid_slot_frames_per_sec": n_lgs * lgs.n_sub ** 2 * K / t_wfs,
                 "hbm_peak_gbs": pk["hbm_gbs"], "hbm_peak_source": pk["source"]}
 
+    # ---- optional: the residual-phase entry (NEXT-2), HBM-bound: every mode array is read once ----
+    dm = None
+    if args.dm_modes > 0:
+        n_el = lgs.n_sub * lgs.n_samp
+        n_el *= n_el
+        modes = torch.randn((args.dm_modes, n_el), dtype=torch.float32, device=dev)
+        coeffs = torch.randn((args.dm_modes,), dtype=torch.float32, device=dev)
+        dmap = torch.empty((n_el,), dtype=torch.float32, device=dev)
+        reps = 10
+        geo.modes_to_map(modes, coeffs, -1.0, dmap)
+        t_dm, _ = timed(lambda: [geo.modes_to_map(modes, coeffs, -1.0, dmap) for _ in range(reps)])
+        nbytes = (args.dm_modes + 1) * n_el * 4.0
+        dm = {"modes": args.dm_modes, "elems": n_el, "us_per_call": 1e6 * t_dm / reps, "bound": "hbm",
+              "achieved": nbytes * reps / t_dm / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+              "frac": nbytes * reps / t_dm / 1e9 / pk["hbm_gbs"]}
+        del modes
+
     # ---- end to end through the host-buffer entry point (screens uploaded inside the region) ----
     e2e = None
     if not args.skip_e2e:
@@ -313,6 +330,8 @@ def run_gpu(args):
                            "parallelism": f"steps split over {world} GPU(s), screens replicated"},
                 "clocks": clocks, "gpu_launches": launches, "roofline": roofline, "e2e": e2e,
                 "cpu_baseline": cpu, "setup_seconds": t_setup}
+        if dm is not None:
+            line["dm_modes"] = dm
         print(json.dumps(line))
     geo.close()
     return 0
@@ -335,6 +354,7 @@ def main():
     ap.add_argument("--batch", type=int, default=50, help="time steps per C-ABI call")
     ap.add_argument("--serial", action="store_true", help="one C-ABI call per leg on one stream instead of ao_forward")
     ap.add_argument("--phase-maps", action="store_true", help="set a static additive phase map on every source (ao_set_phase_map)")
+    ap.add_argument("--dm-modes", type=int, default=0, help="also time ao_modes_to_map with this many modes on the LGS grid")
     ap.add_argument("--skip-e2e", action="store_true")
     ap.add_argument("--skip-cpu", action="store_true")
     args = ap.parse_args()
