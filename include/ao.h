@@ -193,6 +193,15 @@ int ao_set_phase_map(ao_geometry* g, int source, const float* map_dev);
 int ao_modes_to_map(ao_geometry* g, const float* modes_dev, int n_modes, long long n_elems,
                     const float* coeffs_dev, float sign, float* map_dev, void* cuda_stream);
 
+/* ao_strehl -- Strehl ratio of every science direction from its long-exposure PSF (section 2.8: "the
+ * Strehl Ratio ... computed on the PSF"): with the PSF normalisation of ao_psf (sum = 1 per exposure) the
+ * diffraction-limited peak is peak_flat = (sum A)^2 / (M^2 sum A^2), at pixel [M/2][M/2], and
+ *   strehl[d] = psf_dev[d][M/2][M/2] / (n_exposures * peak_flat).
+ * psf_dev: [n_sci][M][M] as written by ao_psf / ao_forward; n_exposures: the number of steps summed into it;
+ * strehl_dev: [n_sci] fp32 DEVICE pointer.  Asynchronous on cuda_stream.
+ * Errors: AO_ERR_INVALID_ARG (NULL pointers, n_exposures <= 0, no science direction / psf_fft == 0). */
+int ao_strehl(ao_geometry* g, const float* psf_dev, double n_exposures, float* strehl_dev, void* cuda_stream);
+
 /* ao_forward -- the whole step with DEVICE buffers: ray-trace + every WFS (slopes only, noiseless unless
  * `noise`) + every science PSF for n_steps steps (the per-time-step forward model).
  * Same results as one ao_sh_images(phase_dev = NULL, images_dev = NULL) per WFS plus ao_psf(phase_dev = NULL),

@@ -172,6 +172,15 @@ def noise(images: np.ndarray, valid, seed: int, source: int, step: int, photons:
 
 
 # ------------------------------------------------------------------------------- step driver
+def strehl(psf_sum: np.ndarray, amp: np.ndarray, n_exposures: float) -> float:
+    """Strehl ratio on the PSF (section 2.8): peak pixel [M/2][M/2] of the long exposure over n_exposures times
+    the diffraction-limited peak (sum A)^2 / (M^2 sum A^2) of the PSF normalisation of reading O7.  FP64."""
+    M = psf_sum.shape[0]
+    a = np.asarray(amp, dtype=np.float64)
+    peak_flat = a.sum() ** 2 / (M * M * (a * a).sum())
+    return float(psf_sum[M // 2, M // 2] / (n_exposures * peak_flat))
+
+
 def modes_to_map(modes: np.ndarray, coeffs: np.ndarray, sign: float) -> np.ndarray:
     """Residual-phase entry (PAPER.md:82 section 2.7, :74 section 2.5): map = sign * sum_m coeffs[m] modes[m], FP64.
     The plain definition: one numpy contraction over the mode index."""

@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "AO_OK", 1: "AO_ERR_INVALID_ARG", 2: "AO_ERR_SHAPE", 3: "AO_E
 # every symbol include/ao.h declares
 EXPORTS = ["ao_geometry_create", "ao_geometry_destroy", "ao_workspace_bytes", "ao_set_workspace",
            "ao_phase_elems_per_step", "ao_phase_offset", "ao_wfs_valid", "ao_trace_layers",
-           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_phase_map", "ao_modes_to_map", "ao_forward", "ao_forward_host", "ao_launch_count",
+           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_phase_map", "ao_modes_to_map", "ao_strehl", "ao_forward", "ao_forward_host", "ao_launch_count",
            "ao_last_error", "ao_version"]
 
 
@@ -84,6 +84,7 @@ def load_library():
     L.ao_psf.argtypes = [vp, vp, i64, i32, dbl, vp, i32, vp]
     L.ao_set_phase_map.argtypes = [vp, i32, vp]
     L.ao_modes_to_map.argtypes = [vp, vp, i32, i64, vp, C.c_float, vp, vp]
+    L.ao_strehl.argtypes = [vp, vp, dbl, vp, vp]
     L.ao_forward.argtypes = [vp, i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, i32, vp]
     L.ao_forward_host.argtypes = [vp, C.POINTER(vp), i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, vp]
     L.ao_launch_count.argtypes = [vp]; L.ao_launch_count.restype = i64
@@ -267,6 +268,13 @@ class Geometry:
             psf = torch.zeros((n_sci, M, M), dtype=torch.float32, device=self.device)
         _check(self.lib.ao_psf(self.handle, _ptr(phase), step0, n_steps, dt_s, _ptr(psf), int(accumulate), _stream()))
         return psf
+
+    def strehl(self, psf, n_exposures: float):
+        """ao_strehl: [n_sci] Strehl ratios of a long-exposure PSF summed over n_exposures steps."""
+        import torch
+        out = torch.empty((len(self.cfg.science_sources()),), dtype=torch.float32, device=self.device)
+        _check(self.lib.ao_strehl(self.handle, _ptr(psf), float(n_exposures), _ptr(out), _stream()))
+        return out
 
     def forward(self, step0: int, n_steps: int, dt_s: float, slopes: Sequence, psf=None, accumulate=False, noise=None):
         """ao_forward: every WFS (slopes[w] device tensors, None to skip) and the science PSF in one call."""

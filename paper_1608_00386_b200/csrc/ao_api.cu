@@ -285,7 +285,7 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
 
     g->Np = pupil->n; g->pitch = pupil->pitch_m; g->lambda_ref = lambda_ref_m;
     const size_t np2 = (size_t)g->Np * g->Np;
-    for (size_t i = 0; i < np2; ++i) g->sumA2 += (double)pupil->amp_host[i] * pupil->amp_host[i];
+    for (size_t i = 0; i < np2; ++i) { g->sumA2 += (double)pupil->amp_host[i] * pupil->amp_host[i]; g->sumA += (double)pupil->amp_host[i]; }
     if ((e = upload(&g->d_pupil_amp, pupil->amp_host, np2)) != cudaSuccess) return bail("pupil upload");
 
     const double PI = 3.14159265358979323846;
@@ -555,6 +555,18 @@ int ao_modes_to_map(ao_geometry* g, const float* modes_dev, int n_modes, long lo
     if (n_modes < 0 || n_elems < 0) return fail(AO_ERR_INVALID_ARG, "ao_modes_to_map: negative size");
     if (!map_dev || (n_modes > 0 && (!modes_dev || !coeffs_dev))) return fail(AO_ERR_INVALID_ARG, "ao_modes_to_map: NULL pointer");
     AO_CUDA(launch_modes_to_map(g, modes_dev, n_modes, n_elems, coeffs_dev, sign, map_dev, (cudaStream_t)cuda_stream), "modes_to_map");
+    return AO_OK;
+}
+
+int ao_strehl(ao_geometry* g, const float* psf_dev, double n_exposures, float* strehl_dev, void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (g->sci.src.empty() || !g->psf_fft) return fail(AO_ERR_INVALID_ARG, "ao_strehl: no science direction / psf_fft == 0");
+    if (!psf_dev || !strehl_dev || !(n_exposures > 0.0)) return fail(AO_ERR_INVALID_ARG, "ao_strehl: NULL pointer or n_exposures <= 0");
+    const double M = (double)g->psf_fft;
+    const double peak_flat = g->sumA2 > 0 ? g->sumA * g->sumA / (M * M * g->sumA2) : 0.0;
+    const float inv = peak_flat > 0 ? (float)(1.0 / (n_exposures * peak_flat)) : 0.0f;
+    AO_CUDA(launch_strehl(g, psf_dev, (int)g->sci.src.size(), g->psf_fft, inv, strehl_dev, (cudaStream_t)cuda_stream), "strehl");
     return AO_OK;
 }
 

@@ -74,7 +74,7 @@ struct ao_geometry {
     int Np = 0;
     double pitch = 0;
     float* d_pupil_amp = nullptr;
-    double sumA2 = 0;
+    double sumA2 = 0, sumA = 0;
     std::vector<ao::WfsH> wfs;
     std::vector<ao::LayerP> layers;
     ao::LayerP* d_layers = nullptr;
@@ -112,6 +112,8 @@ cudaError_t launch_centroids(ao_geometry* g, const WfsH& w, const float* images,
 
 cudaError_t launch_modes_to_map(ao_geometry* g, const float* modes, int n_modes, long long n_elems, const float* coeffs,
                                 float sign, float* map, cudaStream_t st);
+
+cudaError_t launch_strehl(ao_geometry* g, const float* psf, int n_dir, int M, float inv_norm, float* strehl, cudaStream_t st);
 
 cudaError_t launch_noise(ao_geometry* g, const WfsH& w, float* images, int64_t step0, int n_steps,
                          const NoiseP& noise, cudaStream_t st);

@@ -240,6 +240,21 @@ cudaError_t launch_modes_to_map(ao_geometry* g, const float* modes, int n_modes,
 }
 
 // ------------------------------------------------------------------------------------------
+// ao_strehl: peak pixel [M/2][M/2] of every long-exposure PSF over the diffraction-limited peak.
+__global__ void k_strehl(const float* __restrict__ psf, int n_dir, int M, float inv_norm, float* __restrict__ strehl)
+{
+    const int d = blockIdx.x * blockDim.x + threadIdx.x;
+    if (d < n_dir) strehl[d] = psf[((size_t)d * M + M / 2) * M + M / 2] * inv_norm;
+}
+
+cudaError_t launch_strehl(ao_geometry* g, const float* psf, int n_dir, int M, float inv_norm, float* strehl, cudaStream_t st)
+{
+    k_strehl<<<(n_dir + 63) / 64, 64, 0, st>>>(psf, n_dir, M, inv_norm, strehl);
+    g->launches++;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
 // Stand-alone detector noise, in place on [n_steps][n_sel][nsa][P][P] normalised images.
 __global__ void __launch_bounds__(256)
 k_noise(float* __restrict__ images, const uint8_t* __restrict__ valid, const int* __restrict__ sel,

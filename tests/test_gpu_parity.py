@@ -444,3 +444,25 @@ def test_modes_to_map_and_closed_loop_residual():
     geo.modes_to_map(None, None, 1.0, d_map)                  # no modes: zero map
     torch.cuda.synchronize()
     assert float(d_map.abs().max()) == 0.0
+
+
+def test_strehl_on_the_long_exposure_psf():
+    """ao_strehl (PAPER.md:86): peak of the long-exposure PSF over the diffraction-limited peak, against the oracle;
+    a flat atmosphere gives Strehl 1 in every science direction."""
+    import torch
+    cfg = inputs.make_config(3, n_sub=8, screen_n=512, n_steps=3)
+    geo = _geo(cfg, 3)
+    psf = geo.psf(None, 0, 3, cfg.dt_s)
+    got = geo.strehl(psf, 3).cpu().numpy()
+    ref = oracle.forward(cfg, 0, 3, want_phase=False, want_wfs=False)
+    want = np.array([oracle.strehl(ref["psf"][s], cfg.pupil.amp, 3) for s in cfg.science_sources()])
+    assert got.shape == want.shape and np.abs(got - want).max() <= 1e-5 * max(1.0, np.abs(want).max())
+    assert (want < 0.9).all()                                  # the turbulence does degrade the image
+    for lay in cfg.layers:
+        lay.screen = np.zeros_like(lay.screen)
+    flat = _geo(cfg, 1)
+    s1 = flat.strehl(flat.psf(None, 0, 1, cfg.dt_s), 1).cpu().numpy()
+    assert np.abs(s1 - 1.0).max() <= 1e-5
+    from paper_1608_00386_b200 import binding
+    with pytest.raises(binding.AoError):
+        flat.strehl(psf, 0)                                    # n_exposures must be positive

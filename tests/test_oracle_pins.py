@@ -632,3 +632,21 @@ def test_residual_of_a_tilt_mode_cancels_a_tilted_wavefront():
     cfg.phase_maps = {0: oracle.modes_to_map(mode, np.array([alpha]), -1.0)}
     closed = oracle.forward(cfg, 0, 1)
     assert np.abs(closed["slopes"][0]).max() < 1e-9
+
+
+# ----------------------------------------------------------------------------- Strehl on the PSF
+def test_strehl_flat_is_one_tilt_is_zero_and_marechal_for_small_aberrations():
+    N, M = 48, 128
+    amp = inputs.annulus_mask(N, 0.1, 2.4, 0.7)
+    flat = oracle.psf(np.zeros((N, N)), amp, M)
+    assert abs(oracle.strehl(flat, amp, 1) - 1.0) < 1e-12                       # diffraction limit
+    assert abs(oracle.strehl(3.0 * flat, amp, 3) - 1.0) < 1e-12                 # long exposure of 3 equal steps
+    tilt = np.tile(2.0 * np.pi * 8 * np.arange(N) / M, (N, 1))                  # spot moved 8 pixels away: peak pixel ~ empty
+    assert oracle.strehl(oracle.psf(tilt, amp, M), amp, 1) < 1e-3
+    rng = np.random.default_rng(4)
+    for sigma in (0.05, 0.1, 0.2):                                              # Marechal: S = exp(-sigma^2) + O(sigma^4 / N_lit)
+        ph = rng.normal(scale=sigma, size=(N, N))
+        lit = amp > 0
+        var = ph[lit].var()
+        s = oracle.strehl(oracle.psf(ph, amp, M), amp, 1)
+        assert abs(s - np.exp(-var)) < 0.02 * var + 1e-4, (sigma, s, np.exp(-var))
