@@ -202,6 +202,14 @@ int ao_modes_to_map(ao_geometry* g, const float* modes_dev, int n_modes, long lo
  * Errors: AO_ERR_INVALID_ARG (NULL pointers, n_exposures <= 0, no science direction / psf_fft == 0). */
 int ao_strehl(ao_geometry* g, const float* psf_dev, double n_exposures, float* strehl_dev, void* cuda_stream);
 
+/* ao_strehl_marechal -- Strehl ratio by the Marechal approximation on the wavefront (section 2.8: "or
+ * by the Marechal approximation on the closed loop WF"):  strehl[k][d] = exp(-var_A(phi_{k,d})), var_A the
+ * amplitude-weighted variance of the phase of science direction d over the pupil (weights A[i][j], piston removed),
+ * accumulated in FP64.  phase_dev: ao_trace_layers layout (radians at each source's wavelength; residual phase if
+ * maps are set), n_steps steps; strehl_dev: [n_steps][n_sci] fp32 DEVICE pointer.  Asynchronous on cuda_stream.
+ * Errors: AO_ERR_INVALID_ARG (NULL pointers, n_steps < 0, no science direction). */
+int ao_strehl_marechal(ao_geometry* g, const float* phase_dev, int n_steps, float* strehl_dev, void* cuda_stream);
+
 /* ao_forward -- the whole step with DEVICE buffers: ray-trace + every WFS (slopes only, noiseless unless
  * `noise`) + every science PSF for n_steps steps (the per-time-step forward model).
  * Same results as one ao_sh_images(phase_dev = NULL, images_dev = NULL) per WFS plus ao_psf(phase_dev = NULL),

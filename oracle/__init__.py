@@ -181,6 +181,15 @@ def strehl(psf_sum: np.ndarray, amp: np.ndarray, n_exposures: float) -> float:
     return float(psf_sum[M // 2, M // 2] / (n_exposures * peak_flat))
 
 
+def strehl_marechal(phase: np.ndarray, amp: np.ndarray) -> float:
+    """Marechal approximation (section 2.8): exp(-var_A(phi)), the amplitude-weighted phase variance over
+    the pupil with the weighted mean (piston) removed.  FP64, the definition written out."""
+    w = np.asarray(amp, dtype=np.float64)
+    p = np.asarray(phase, dtype=np.float64)
+    mean = (w * p).sum() / w.sum()
+    return float(np.exp(-(w * (p - mean) ** 2).sum() / w.sum()))
+
+
 def modes_to_map(modes: np.ndarray, coeffs: np.ndarray, sign: float) -> np.ndarray:
     """Residual-phase entry (PAPER.md:82 section 2.7, :74 section 2.5): map = sign * sum_m coeffs[m] modes[m], FP64.
     The plain definition: one numpy contraction over the mode index."""

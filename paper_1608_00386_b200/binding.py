@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "AO_OK", 1: "AO_ERR_INVALID_ARG", 2: "AO_ERR_SHAPE", 3: "AO_E
 # every symbol include/ao.h declares
 EXPORTS = ["ao_geometry_create", "ao_geometry_destroy", "ao_workspace_bytes", "ao_set_workspace",
            "ao_phase_elems_per_step", "ao_phase_offset", "ao_wfs_valid", "ao_trace_layers",
-           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_phase_map", "ao_modes_to_map", "ao_strehl", "ao_forward", "ao_forward_host", "ao_launch_count",
+           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_phase_map", "ao_modes_to_map", "ao_strehl", "ao_strehl_marechal", "ao_forward", "ao_forward_host", "ao_launch_count",
            "ao_last_error", "ao_version"]
 
 
@@ -85,6 +85,7 @@ def load_library():
     L.ao_set_phase_map.argtypes = [vp, i32, vp]
     L.ao_modes_to_map.argtypes = [vp, vp, i32, i64, vp, C.c_float, vp, vp]
     L.ao_strehl.argtypes = [vp, vp, dbl, vp, vp]
+    L.ao_strehl_marechal.argtypes = [vp, vp, i32, vp, vp]
     L.ao_forward.argtypes = [vp, i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, i32, vp]
     L.ao_forward_host.argtypes = [vp, C.POINTER(vp), i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, vp]
     L.ao_launch_count.argtypes = [vp]; L.ao_launch_count.restype = i64
@@ -274,6 +275,13 @@ class Geometry:
         import torch
         out = torch.empty((len(self.cfg.science_sources()),), dtype=torch.float32, device=self.device)
         _check(self.lib.ao_strehl(self.handle, _ptr(psf), float(n_exposures), _ptr(out), _stream()))
+        return out
+
+    def strehl_marechal(self, phase, n_steps: int):
+        """ao_strehl_marechal: [n_steps][n_sci] exp(-weighted phase variance) from an ao_trace_layers phase buffer."""
+        import torch
+        out = torch.empty((n_steps, len(self.cfg.science_sources())), dtype=torch.float32, device=self.device)
+        _check(self.lib.ao_strehl_marechal(self.handle, _ptr(phase), int(n_steps), _ptr(out), _stream()))
         return out
 
     def forward(self, step0: int, n_steps: int, dt_s: float, slopes: Sequence, psf=None, accumulate=False, noise=None):

@@ -570,6 +570,15 @@ int ao_strehl(ao_geometry* g, const float* psf_dev, double n_exposures, float* s
     return AO_OK;
 }
 
+int ao_strehl_marechal(ao_geometry* g, const float* phase_dev, int n_steps, float* strehl_dev, void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (g->sci.src.empty()) return fail(AO_ERR_INVALID_ARG, "ao_strehl_marechal: no science direction");
+    if (!phase_dev || !strehl_dev || n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_strehl_marechal: NULL pointer or n_steps < 0");
+    AO_CUDA(launch_marechal(g, phase_dev, g->phase_elems_per_step, n_steps, strehl_dev, (cudaStream_t)cuda_stream), "marechal");
+    return AO_OK;
+}
+
 int ao_forward(ao_geometry* g, int64_t step0, int n_steps, double dt_s, const ao_noise* noise,
                float* const* slopes_dev, float* psf_dev, int accumulate, void* cuda_stream)
 {

@@ -115,6 +115,9 @@ cudaError_t launch_modes_to_map(ao_geometry* g, const float* modes, int n_modes,
 
 cudaError_t launch_strehl(ao_geometry* g, const float* psf, int n_dir, int M, float inv_norm, float* strehl, cudaStream_t st);
 
+cudaError_t launch_marechal(ao_geometry* g, const float* phase, long long step_stride, int n_steps, float* strehl,
+                            cudaStream_t st);
+
 cudaError_t launch_noise(ao_geometry* g, const WfsH& w, float* images, int64_t step0, int n_steps,
                          const NoiseP& noise, cudaStream_t st);
 

@@ -255,6 +255,47 @@ cudaError_t launch_strehl(ao_geometry* g, const float* psf, int n_dir, int M, fl
 }
 
 // ------------------------------------------------------------------------------------------
+// ao_strehl_marechal: exp(-amplitude-weighted phase variance) per (step, science direction); one CTA each, FP64 sums
+// of w, w phi, w phi^2 (phase is tens of radians in open loop: the difference of squares needs the headroom).
+__global__ void __launch_bounds__(256)
+k_marechal(const float* __restrict__ phase, long long step_stride, const long long* __restrict__ off, int n_dir,
+           const float* __restrict__ amp, int N, float* __restrict__ strehl)
+{
+    __shared__ double red[3][8];
+    const int d = blockIdx.x % n_dir, k = blockIdx.x / n_dir;
+    const float* ph = phase + (size_t)k * step_stride + off[d];
+    double sw = 0.0, s1 = 0.0, s2 = 0.0;
+    for (size_t i = threadIdx.x; i < (size_t)N * N; i += 256) {
+        const double w = (double)amp[i], p = (double)ph[i];
+        sw += w; s1 += w * p; s2 += w * p * p;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        sw += __shfl_xor_sync(0xffffffffu, sw, o); s1 += __shfl_xor_sync(0xffffffffu, s1, o); s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) { red[0][warp] = sw; red[1][warp] = s1; red[2][warp] = s2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        sw = s1 = s2 = 0.0;
+        for (int w = 0; w < 8; ++w) { sw += red[0][w]; s1 += red[1][w]; s2 += red[2][w]; }
+        double var = 0.0;
+        if (sw > 0.0) { const double mean = s1 / sw; var = s2 / sw - mean * mean; if (var < 0.0) var = 0.0; }
+        strehl[blockIdx.x] = (float)exp(-var);
+    }
+}
+
+cudaError_t launch_marechal(ao_geometry* g, const float* phase, long long step_stride, int n_steps, float* strehl,
+                            cudaStream_t st)
+{
+    const int n_dir = (int)g->sci.src.size();
+    if (n_dir == 0 || n_steps <= 0) return cudaSuccess;
+    k_marechal<<<(unsigned)(n_dir * n_steps), 256, 0, st>>>(phase, step_stride, g->sci.d_off_api, n_dir, g->d_pupil_amp,
+                                                            g->Np, strehl);
+    g->launches++;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
 // Stand-alone detector noise, in place on [n_steps][n_sel][nsa][P][P] normalised images.
 __global__ void __launch_bounds__(256)
 k_noise(float* __restrict__ images, const uint8_t* __restrict__ valid, const int* __restrict__ sel,

@@ -466,3 +466,22 @@ def test_strehl_on_the_long_exposure_psf():
     from paper_1608_00386_b200 import binding
     with pytest.raises(binding.AoError):
         flat.strehl(psf, 0)                                    # n_exposures must be positive
+
+
+def test_marechal_strehl_on_traced_phase():
+    """ao_strehl_marechal on the ao_trace_layers buffer against the oracle, with a residual-phase map on
+    one science direction; open-loop phase variances are hundreds of rad^2, so compare the exponent too."""
+    import torch
+    cfg = inputs.make_config(3, n_sub=8, screen_n=512, n_steps=2)
+    sci = cfg.science_sources()
+    for lay in cfg.layers:                                   # weak turbulence: Strehl values of order 0.1 - 0.9
+        lay.screen = (0.3 * lay.screen).astype(np.float32)
+    cfg.phase_maps = {sci[1]: _smooth_map(np.random.default_rng(3), cfg.grid_n(sci[1]), 0.3)}
+    geo = _geo(cfg, 2)
+    phase = geo.trace_layers(5, 2, cfg.dt_s)
+    got = geo.strehl_marechal(phase, 2).cpu().numpy().astype(np.float64)
+    ref = oracle.forward(cfg, 5, 2, want_wfs=False, want_psf=False, sources=sci)
+    want = np.array([[oracle.strehl_marechal(ref["phase"][s][k], cfg.pupil.amp) for s in sci] for k in range(2)])
+    assert got.shape == want.shape
+    assert np.abs(got - want).max() <= 1e-5
+    assert (want > 0.01).all() and (want < 0.99).all(), want       # neither saturated nor trivial

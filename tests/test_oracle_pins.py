@@ -650,3 +650,18 @@ def test_strehl_flat_is_one_tilt_is_zero_and_marechal_for_small_aberrations():
         var = ph[lit].var()
         s = oracle.strehl(oracle.psf(ph, amp, M), amp, 1)
         assert abs(s - np.exp(-var)) < 0.02 * var + 1e-4, (sigma, s, np.exp(-var))
+
+
+def test_marechal_strehl_closed_forms_and_agreement_with_the_psf_strehl():
+    N, M = 48, 128
+    amp = inputs.annulus_mask(N, 0.1, 2.4, 0.7)
+    assert oracle.strehl_marechal(np.full((N, N), 7.5), amp) == 1.0             # piston only
+    two = np.where(np.arange(N)[None, :] < N // 2, -0.3, 0.3) * np.ones((N, 1))  # two-level phase +-a on a symmetric pupil
+    assert abs(oracle.strehl_marechal(two, amp) - np.exp(-0.09)) < 1e-12          # variance a^2
+    # outside the pupil the phase does not count
+    junk = two + 100.0 * (amp == 0)
+    assert abs(oracle.strehl_marechal(junk, amp) - np.exp(-0.09)) < 1e-12
+    rng = np.random.default_rng(6)
+    ph = rng.normal(scale=0.15, size=(N, N))
+    s_psf = oracle.strehl(oracle.psf(ph, amp, M), amp, 1)
+    assert abs(oracle.strehl_marechal(ph, amp) - s_psf) < 2e-3                    # the two estimates of PAPER.md:86 agree
