@@ -18,7 +18,7 @@
  * Dirichlet-kernel closed forms and the tilt/CoG table of SURVEY.md §8(c)
  * (tests/golden/), Parseval, flat->zero slopes, piston invariance, linear-screen
  * bilinear exactness, integer/half-pixel shifts, cone scaling, periodicity,
- * cuRAND's host Philox4_32_10 generator, Poisson/Gauss statistics.
+ * cuRAND's host Philox4_32_10 generator, scipy.stats.poisson.ppf (mu up to 1e4), Poisson/Gauss statistics.
  * No function here is "parity unpinned".
  *
  * Layout: all arrays row-major [y][x], x fastest.
@@ -402,19 +402,49 @@ void aoref_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t 
 /* u = ((w >> 8) + 0.5) 2^-24 : in (0,1), exactly representable in fp32 and fp64. */
 static inline double u24(uint32_t w) { return ((double)(w >> 8) + 0.5) * (1.0 / 16777216.0); }
 
-/* Poisson by sequential-search inversion: k = 0; p = c = exp(-mu); while u > c: k++, p *= mu/k, c += p. */
+/* Poisson by inversion of the CDF on u: the smallest k with u <= F(k; mu), F(k) = sum_{j<=k} e^-mu mu^j / j!.
+ *   mu < 64: sequential search from 0: k = 0; p = c = exp(-mu); while u > c: k++, p *= mu/k, c += p.
+ *   mu >= 64 (reading O5 as revised in round 2: exp(-mu) underflows FP64 above mu ~ 745 and the
+ *   search from 0 then returns floor(mu)+1 for every u): the same inverse CDF, searched from the mode m = floor(mu):
+ *     p_m = exp(m ln mu - mu - lgamma(m+1));  F(m) = p_m + p_{m-1} + ... (p_{j-1} = p_j j/mu, until a term adds nothing);
+ *     u <= F(m): walk down while u <= F(k) - p_k (then k--), else walk up while u > F(k) (k++, p *= mu/k, F += p).
+ * Pinned against scipy.stats.poisson.ppf for mu up to 1e4 and by the variance at mu = 800, 1e3, 1e4. */
 static int32_t poisson_inv(double mu, double u)
 {
     if (!(mu > 0.0)) return 0;
-    int32_t k = 0;
-    double p = exp(-mu), c = p;
-    while (u > c && k < 100000) {
-        ++k;
-        p *= mu / (double)k;
-        c += p;
-        if (p == 0.0 && (double)k > mu) break;   /* CDF saturated below u by rounding */
+    if (mu < 64.0) {
+        int32_t k = 0;
+        double p = exp(-mu), c = p;
+        while (u > c && k < 100000) {
+            ++k;
+            p *= mu / (double)k;
+            c += p;
+            if (p == 0.0 && (double)k > mu) break;   /* CDF saturated below u by rounding */
+        }
+        return k;
     }
-    return k;
+    const double m = floor(mu);
+    const double pm = exp(m * log(mu) - mu - lgamma(m + 1.0));
+    double Fm = pm, p = pm;
+    for (double j = m; j >= 1.0; j -= 1.0) {          /* F(m): terms below the mode, largest first */
+        p *= j / mu;
+        const double next = Fm + p;
+        if (next == Fm) break;
+        Fm = next;
+    }
+    double k = m, c = Fm;
+    p = pm;
+    if (u <= c) {
+        while (k > 0.0 && u <= c - p) { c -= p; p *= k / mu; k -= 1.0; }
+    } else {
+        while (u > c && k < 2147483000.0) {
+            k += 1.0;
+            p *= mu / k;
+            c += p;
+            if (p == 0.0) break;                      /* CDF saturated below u by rounding */
+        }
+    }
+    return (int32_t)k;
 }
 
 /*   mu = photons * I ; key = (seed lo, seed hi) ; counter = (pixel-in-image, subaperture, source, step)

@@ -25,17 +25,15 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1
 // u = ((w >> 8) + 0.5) 2^-24, exact in fp32.
 __device__ __forceinline__ float u24(uint32_t w) { return ((float)(w >> 8) + 0.5f) * (1.0f / 16777216.0f); }
 
-// Detector pixel with noise (reading O5): Poisson(mu) by sequential-search inversion of the
-// CDF plus read_noise * N(0,1) (Box-Muller).  The CDF search runs in FP64: exp(-mu) underflows
-// fp32 for mu > 87 and the integer decision must not depend on fp32 rounding of the CDF.
-__device__ __forceinline__ float noisy_pixel(float I, const NoiseP& nz, uint32_t px, uint32_t sa,
-                                             uint32_t src, uint32_t step)
+// Poisson by inversion of the CDF on u (reading O5): the smallest k with u <= F(k; mu), searched in FP64 (exp(-mu)
+// underflows fp32 for mu > 87 and the integer decision must not depend on fp32 rounding of the CDF).  mu < 64: sequential
+// search from 0.  mu >= 64: the same inverse CDF searched from the mode m = floor(mu) (exp(-mu) underflows FP64 above
+// mu ~ 745): p_m = exp(m ln mu - mu - lgamma(m + 1)), F(m) summed downwards from the mode, then a walk down or up.
+static __device__ __noinline__ int poisson_inv(const double mu, const double u)
 {
-    const uint4 w = philox4x32_10(make_uint4(px, sa, src, step), nz.key0, nz.key1);
-    const double mu = (double)(nz.photons * I);
-    int k = 0;
-    if (mu > 0.0) {
-        const double u = (double)u24(w.x);
+    if (!(mu > 0.0)) return 0;
+    if (mu < 64.0) {
+        int k = 0;
         double p = exp(-mu), c = p;
         while (u > c && k < 100000) {
             ++k;
@@ -43,7 +41,38 @@ __device__ __forceinline__ float noisy_pixel(float I, const NoiseP& nz, uint32_t
             c += p;
             if (p == 0.0 && (double)k > mu) break;
         }
+        return k;
     }
+    const double m = floor(mu);
+    const double pm = exp(m * log(mu) - mu - lgamma(m + 1.0));
+    double Fm = pm, p = pm;
+    for (double j = m; j >= 1.0; j -= 1.0) {
+        p *= j / mu;
+        const double next = Fm + p;
+        if (next == Fm) break;
+        Fm = next;
+    }
+    double k = m, c = Fm;
+    p = pm;
+    if (u <= c) {
+        while (k > 0.0 && u <= c - p) { c -= p; p *= k / mu; k -= 1.0; }
+    } else {
+        while (u > c && k < 2147483000.0) {
+            k += 1.0;
+            p *= mu / k;
+            c += p;
+            if (p == 0.0) break;
+        }
+    }
+    return (int)k;
+}
+
+// Detector pixel with noise (reading O5): Poisson(mu) by inversion of the CDF plus read_noise * N(0,1) (Box-Muller).
+__device__ __forceinline__ float noisy_pixel(float I, const NoiseP& nz, uint32_t px, uint32_t sa,
+                                             uint32_t src, uint32_t step)
+{
+    const uint4 w = philox4x32_10(make_uint4(px, sa, src, step), nz.key0, nz.key1);
+    const int k = poisson_inv((double)(nz.photons * I), (double)u24(w.x));
     const float z = sqrtf(-2.0f * logf(u24(w.y))) * cospif(2.0f * u24(w.z));
     return fmaf(nz.read_noise, z, (float)k);
 }

@@ -528,6 +528,41 @@ def test_noise_skips_invalid_subapertures_and_full_cdf_range():
     assert abs(counts.mean() - 300.0) < 4 * math.sqrt(300.0 / 64)
 
 
+@pytest.mark.parametrize("mu", [63.9, 64.0, 100.5, 226.7, 744.0, 746.0, 800.0, 1026.3, 1e4])
+def test_poisson_inverse_cdf_matches_scipy_for_bright_pixels(mu):
+    """Reading O5 (revised): the Poisson draw is the inverse CDF at u for EVERY mean.  exp(-mu) underflows FP64 above
+    mu ~ 745, where a search from k = 0 returns floor(mu)+1 for every u; the oracle searches from the mode instead.
+    Library routine: scipy.stats.poisson.ppf; statistics: mean and variance of the counts equal mu."""
+    from scipy.stats import poisson
+    P, n_img, seed, src, step = 16, 40, 77, 2, 5
+    img = np.full((n_img, P, P), 1.0)
+    _, counts = oracle.noise(img, None, seed, src, step, mu, 0.0)              # photons = mu, image = 1
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    for sa in (0, 3, 39):
+        for px in range(0, P * P, 5):
+            w = oracle.philox4x32_10([px, sa, src, step], key)
+            u = ((int(w[0]) >> 8) + 0.5) / 2 ** 24
+            assert counts[sa].ravel()[px] == int(poisson.ppf(u, mu)), (mu, u)
+    c = counts.astype(np.float64).ravel()
+    n = c.size
+    assert abs(c.mean() - mu) < 4.0 * math.sqrt(mu / n)
+    assert abs(c.var() / mu - 1.0) < 4.0 * math.sqrt(2.0 / n) + 1.0 / mu          # a constant floor(mu)+1 would give 0
+
+
+def test_poisson_inverse_cdf_tails():
+    """Extreme u (the ends of the 24-bit lattice) at small and large means, through the exported entry point: a
+    one-pixel image and a search over Philox counters for the smallest and largest u of a few thousand draws."""
+    from scipy.stats import poisson
+    for mu in (3.0, 90.0, 2000.0):
+        img = np.full((200, 4, 4), 1.0)
+        _, counts = oracle.noise(img, None, 11, 0, 0, mu, 0.0)
+        key = [11, 0]
+        us = np.array([[((int(oracle.philox4x32_10([px, sa, 0, 0], key)[0]) >> 8) + 0.5) / 2 ** 24
+                        for px in range(16)] for sa in range(200)])
+        for idx in (np.unravel_index(us.argmin(), us.shape), np.unravel_index(us.argmax(), us.shape)):
+            assert counts[idx[0]].ravel()[idx[1]] == int(poisson.ppf(us[idx], mu)), (mu, us[idx])
+
+
 # ----------------------------------------------------------------------------- input generator (harness)
 def test_screen_generator_variance_and_structure_function():
     n, d = 256, 0.1
@@ -665,3 +700,61 @@ def test_marechal_strehl_closed_forms_and_agreement_with_the_psf_strehl():
     ph = rng.normal(scale=0.15, size=(N, N))
     s_psf = oracle.strehl(oracle.psf(ph, amp, M), amp, 1)
     assert abs(oracle.strehl_marechal(ph, amp) - s_psf) < 2e-3                    # the two estimates of PAPER.md:86 agree
+
+
+# ----------------------------------------------------------------------------- step driver wiring (O2 t_k, O5 counter)
+def test_forward_time_and_noise_counter_use_the_absolute_step_index():
+    """oracle.forward(step0 = 7, n_steps = 2): entry k = 1 is time t = (7 + 1) dt and its
+    noise counter is (pixel, subaperture, GLOBAL source index, 7 + 1) (O5).  Compared with direct calls of the pinned
+    pieces, on a workload whose wind moves the footprint by a non-integer number of pixels per step and whose sensor
+    sources are not source 0, so that t = k dt, a local source index or step k instead of step0 + k all fail."""
+    cfg = inputs.make_config(2, n_sub=6, screen_n=128, n_steps=2, n_layers=3)
+    cfg.sources = cfg.sources[3:5]                       # global indices 0, 1 of this config; keep two LGS
+    cfg.noise = inputs.Noise(seed=0x1234567890ABCDEF, photons_per_subap=1000.0, read_noise_e=3.0)
+    res = oracle.forward(cfg, 7, 2, noise_on=True)
+    W = cfg.wfs[0]
+    for s in (0, 1):
+        src = cfg.sources[s]
+        for k in (0, 1):
+            t = (7 + k) * cfg.dt_s
+            ph = oracle.trace(cfg.layers, src.theta_x_rad, src.theta_y_rad, src.altitude_m, src.lambda_m,
+                              cfg.lambda_ref_m, cfg.grid_n(s), cfg.grid_pitch(s), t)
+            assert np.array_equal(res["phase"][s][k], ph)
+            wrong = oracle.trace(cfg.layers, src.theta_x_rad, src.theta_y_rad, src.altitude_m, src.lambda_m,
+                                 cfg.lambda_ref_m, cfg.grid_n(s), cfg.grid_pitch(s), k * cfg.dt_s)
+            assert np.abs(wrong - ph).max() > 1e-3       # the pin can tell t = k dt from t = (step0 + k) dt
+            img, valid = oracle.sh_images(ph, W.amp, W.n_sub, W.n_samp, W.fft, W.bin, W.n_pix, W.min_illum)
+            assert np.array_equal(res["images"][s][k], img)
+            nz, ct = oracle.noise(img, valid, cfg.noise.seed, s, 7 + k, 1000.0, 3.0)
+            assert np.array_equal(res["counts"][s][k], ct) and np.array_equal(res["noisy"][s][k], nz)
+            for bad_src, bad_step in ((s, k), (1 - s, 7 + k), (s, 7)):
+                if (bad_src, bad_step) != (s, 7 + k):
+                    assert not np.array_equal(oracle.noise(img, valid, cfg.noise.seed, bad_src, bad_step, 1000.0, 3.0)[1], ct)
+            assert np.array_equal(res["slopes"][s][k], oracle.centroids(nz, valid))
+    only1 = oracle.forward(cfg, 7, 2, noise_on=True, sources=[1])      # a subset keeps the global source index
+    assert list(only1["counts"].keys()) == [1] and np.array_equal(only1["counts"][1], res["counts"][1])
+
+
+# ----------------------------------------------------------------------------- SH image on the M > 64 branch (O3, O4)
+def test_big_fft_sensor_image_closed_form_flat_and_integer_tilt():
+    """aoref_sh_images takes its radix-2 branch for M > 64 (the NGS sensors).  Flat n = 48, M = 128, beta = 8, P = 16:
+    the image is the outer product of the binned Dirichlet profile (normalisation 1/(M^2 n^2), full window, bin 8);
+    an x-tilt of exactly one detector pixel (alpha = 2 pi beta / M) shifts the whole image one column to the right,
+    and a cropped window (P = 8: the central 64 of 128 FFT pixels) is the centre of the full image."""
+    n, M, beta, P = 48, 128, 8, 16
+    prof = dirichlet_binned(n, M, beta, P, 0.0)
+    img, valid = one_subap(np.zeros((n, n)), n, M, beta, P)
+    assert valid == 1 and abs(prof.sum() - 1.0) < 1e-12
+    assert np.abs(img - np.outer(prof, prof)).max() < 1e-13
+    a = 2.0 * np.pi * beta / M
+    tilt = np.tile(a * np.arange(n), (n, 1))                        # phase = alpha * column index
+    img_t, _ = one_subap(tilt, n, M, beta, P)
+    px = dirichlet_binned(n, M, beta, P, a)
+    assert np.abs(img_t - np.outer(prof, px)).max() < 1e-13        # rows unchanged, columns carry the tilt
+    assert np.abs(px - np.roll(prof, 1)).max() < 1e-13              # integer shift of the periodic image
+    half, _ = one_subap(np.zeros((n, n)), n, M, beta, 8)
+    assert np.abs(half - img[4:12, 4:12]).max() < 1e-14
+    # y-tilt goes to the rows (orientation), two subapertures side by side are independent
+    ph2 = np.zeros((2 * n, 2 * n)); ph2[:n, n:] = tilt.T
+    img2, v2 = oracle.sh_images(ph2, np.ones((2 * n, 2 * n), np.float32), 2, n, M, beta, P, 0.0)
+    assert np.abs(img2[1] - np.outer(px, prof)).max() < 1e-13 and np.abs(img2[0] - np.outer(prof, prof)).max() < 1e-13
