@@ -21,7 +21,8 @@
  *     (e.g. torch tensors); screens and workspace are borrowed for the life of the handle,
  *     the others for the duration of the call (until the stream work completes).  The library
  *     calls cudaMalloc only inside ao_geometry_create (small tables) and never afterwards.
- *   - A handle is not thread-safe: one handle per host thread / stream.
+ *   - A handle is not thread-safe: one handle per host thread / stream.  It belongs to the CUDA device that was
+ *     current at ao_geometry_create; every compute call makes that device current for the calling thread.
  *   - There is no CPU fallback: without a CUDA device every compute call fails with AO_ERR_CUDA.
  */
 #ifndef AO_H_
@@ -70,8 +71,12 @@ typedef struct {
     double height_m;         /* h_l                                                    */
     double wind_x_mps;       /* the screen moves with +v: the pupil samples x - v t    */
     double wind_y_mps;
-    const float* screen_dev; /* [n][n] radians at lambda_ref, DEVICE pointer, borrowed;
-                                must stay valid and unchanged while the handle is used */
+    const float* screen_dev; /* [n][n] radians at lambda_ref, DEVICE pointer, borrowed; must stay valid while
+                                the handle is used and is only read by the library, with one exception:
+                                ao_forward_host(screens_host != NULL) overwrites it with the host copy, so
+                                for that call the buffer must be writable device memory.  A base address
+                                aligned to 16 bytes with n a multiple of 4 takes the tiled (TMA-staged)
+                                ray-trace; anything else the per-sample fallback kernel (same results) */
 } ao_layer;
 
 /* Guide star or science direction (section 2.2: "all the stars"; LGS at finite distance). */
@@ -97,7 +102,8 @@ typedef struct {
  *   psf_fft      : M of the science PSF (power of two, >= pupil n; 0 if no ao_psf call is made).
  *   out          : receives the handle.
  * Supported sizes: WFS with fft <= 64: any even fft (fast paths for 16/24/32/64);
- *   WFS with fft > 64: fft a power of two <= 4096 and bin*n_pix == fft or smaller central window;
+ *   WFS with fft > 64: fft a power of two <= 4096 and bin*n_pix == fft or smaller central window,
+ *   and (sources using the sensor) x n_sub^2 <= 65535;
  *   psf_fft: power of two in [64, 4096]; n_layers <= 128.  Otherwise AO_ERR_UNSUPPORTED.
  * Errors: AO_ERR_INVALID_ARG (NULL, counts < 0, wfs_index out of range), AO_ERR_SHAPE,
  *   AO_ERR_UNSUPPORTED, AO_ERR_CUDA (no device / allocation failure).  *out is NULL on failure.
@@ -228,7 +234,8 @@ int ao_forward(ao_geometry* g, int64_t step0, int n_steps, double dt_s, const ao
  * ao_sh_images layout; psf_host (nullable) receives [n_sci][M][M] (sum over the steps).
  * The device staging for the results lives in the workspace (see ao_workspace_bytes).
  * If screens_host is non-NULL, screens_host[l] ([S_l][S_l] floats) is first copied into layer
- * l's borrowed device screen (host->device inside the call). */
+ * l's borrowed device screen (host->device inside the call): the one call that writes the screens
+ * (see ao_layer.screen_dev). */
 int ao_forward_host(ao_geometry* g, const float* const* screens_host, int64_t step0, int n_steps,
                     double dt_s, const ao_noise* noise, float* const* slopes_host,
                     float* psf_host, void* cuda_stream);
@@ -237,6 +244,8 @@ int ao_forward_host(ao_geometry* g, const float* const* screens_host, int64_t st
 int64_t ao_launch_count(const ao_geometry* g);
 
 const char* ao_last_error(void);
+/* Version string; it states the build flavour ("normal build", or "PROFILING build" when the library was compiled
+ * with the component-timing switches, whose results are not valid). */
 const char* ao_version(void);
 
 #ifdef __cplusplus

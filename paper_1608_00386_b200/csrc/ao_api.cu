@@ -141,10 +141,17 @@ static NoiseP make_noise(const ao_noise* nz)
     return p;
 }
 
+// Entry check of every compute call: the handle, the device it was created on (made current for this thread
+// if it is not), and errors left by earlier asynchronous work.  The error is only peeked at: errors raised by
+// other libraries in the same process stay theirs to consume.
 static int check_entry(const ao_geometry* g)
 {
     if (!g) return fail(AO_ERR_INVALID_ARG, "NULL handle");
-    cudaError_t e = cudaGetLastError();
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess && dev != g->device) e = cudaSetDevice(g->device);
+    if (e != cudaSuccess) return cuda_fail(e, "selecting the handle's device");
+    e = cudaPeekAtLastError();
     if (e != cudaSuccess) return cuda_fail(e, "pending CUDA error from earlier work");
     return AO_OK;
 }
@@ -227,7 +234,14 @@ using namespace ao;
 extern "C" {
 
 const char* ao_last_error(void) { return g_err.c_str(); }
-const char* ao_version(void) { return "ao-forward-b200 0.1 (sm_100a)"; }
+const char* ao_version(void)
+{
+#ifdef AO_PROFILE_SWITCHES
+    return "ao-forward-b200 0.2 (sm_100a; PROFILING build: AO_DBG component switches compiled in, not for results)";
+#else
+    return "ao-forward-b200 0.2 (sm_100a; normal build)";
+#endif
+}
 
 int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, const ao_layer* layers,
                        int n_layers, const ao_source* src, int n_src, double lambda_ref_m, int psf_fft,
@@ -273,6 +287,7 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
     auto bail = [&](const char* what) { int rc = cuda_fail(e, what); destroy(g); return rc; };
     int dev = 0;
     cudaGetDevice(&dev);
+    g->device = dev;
     cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
     int prio_least = 0, prio_greatest = 0;
     cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest);
@@ -386,6 +401,11 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
     if ((e = build_group(g, g->all)) != cudaSuccess) return bail("group upload");
     if ((e = build_group(g, g->sci)) != cudaSuccess) return bail("group upload");
     for (auto& w : g->wfs) if ((e = build_group(g, w.grp)) != cudaSuccess) return bail("group upload");
+    for (auto& w : g->wfs)      // two-pass FFT sensors put (source, subaperture) on gridDim.y
+        if (w.M > 64 && w.grp.src.size() * (size_t)w.n_sub * w.n_sub > 65535u) {
+            destroy(g);
+            return fail(AO_ERR_UNSUPPORTED, "wfs fft > 64: sources x subapertures of one sensor must not exceed 65535");
+        }
 
     g->psf_fft = psf_fft;
     if (psf_fft) {
@@ -519,23 +539,24 @@ static int forward_chunk(ao_geometry* g, int64_t step0, int n_steps, double dt_s
         AO_CUDA(cudaStreamWaitEvent(g->side, g->ev_fork, 0), "fork wait");
     }
     // the short kernels are submitted first so that they start at once; the long fused launch fills in behind them
-    for (int pass = 0; pass < 2; ++pass) {
-        for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
+    rc = AO_OK;
+    for (int pass = 0; pass < 2 && rc == AO_OK; ++pass) {
+        for (size_t wi = 0; wi < g->wfs.size() && rc == AO_OK; ++wi) {
             const WfsH& w = g->wfs[wi];
             if (!slopes || !slopes[wi] || w.grp.src.empty() || (on_side[wi] != 0) != (pass == 0)) continue;
             rc = run_wfs(g, (int)wi, nullptr, step0, n_steps, dt_s, noise, nullptr, slopes[wi], on_side[wi] ? sw : st);
-            if (rc) return rc;
         }
-        if (pass == 0 && want_psf) {
+        if (pass == 0 && want_psf && rc == AO_OK)
             rc = run_psf(g, nullptr, step0, n_steps, dt_s, psf, accumulate, sw);
-            if (rc) return rc;
-        }
     }
+    // the side stream is joined on every path, also after a failed launch: work already queued there must stay
+    // ordered before whatever the caller submits next on `st`
     if (fork) {
-        AO_CUDA(cudaEventRecord(g->ev_join, g->side), "join record");
-        AO_CUDA(cudaStreamWaitEvent(st, g->ev_join, 0), "join wait");
+        const cudaError_t e1 = cudaEventRecord(g->ev_join, g->side);
+        const cudaError_t e2 = e1 == cudaSuccess ? cudaStreamWaitEvent(st, g->ev_join, 0) : e1;
+        if (e2 != cudaSuccess && rc == AO_OK) return cuda_fail(e2, "join");
     }
-    return AO_OK;
+    return rc;
 }
 
 int ao_set_phase_map(ao_geometry* g, int source, const float* map_dev)

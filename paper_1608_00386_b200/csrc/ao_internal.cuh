@@ -92,7 +92,8 @@ struct ao_geometry {
     int ws_chunk = 0;                 // steps per internal chunk that fit the workspace
     int64_t launches = 0;
     int sm_count = 148;
-    // ao_forward: side stream for the workspace-free sensors, fork / join events
+    int device = 0;                   // the CUDA device the handle was created on (made current by every call)
+    // ao_forward: high-priority side stream for the workspace users (big-FFT sensors, PSF), fork / join events
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };

@@ -449,6 +449,7 @@ cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, boo
     int kb = per_step ? (int)std::min<size_t>(4, scratch_bytes / per_step) : 1;
     if (kb < 1) kb = 1;
     while (kb > 1 && (size_t)kb * per_step > ((size_t)96 << 20)) --kb;
+    while (kb > 1 && (size_t)kb * batch > 65535u) --kb;    // the batch is gridDim.y (ao_geometry_create bounds one step)
     for (int k = 0; k < n_steps; k += kb) {
         const int kn = n_steps - k < kb ? n_steps - k : kb;
         BigRowArgs r;

@@ -114,7 +114,7 @@ k_fused(const FusedArgs A)
     const int g = tid / n, b = tid - g * n;                // subaperture in round, column in subaperture
     float2* xs = xch + (size_t)g * K::SUB_STRIDE;
 #pragma unroll 1
-    for (int rd = (A.T.dbg & 4) ? K::ROUNDS : 0; rd < K::ROUNDS; ++rd) {
+    for (int rd = AO_DBG_ON(A.T, 4) ? K::ROUNDS : 0; rd < K::ROUNDS; ++rd) {
         const int hs = rd >> 1, c = rd & 1;                // hs = step-in-pair * R2 + subaperture row
         const int sp2 = hs / R2, h = hs - sp2 * R2;
         const int k = 2 * kp + sp2;

@@ -34,8 +34,17 @@ struct Trace2Args {
     int pitch;            // staged row pitch in floats (multiple of 4)
     int rows;             // staged rows allocated per stage (box rows + 1 prefetch pad row)
     int ns;               // stages in flight
-    int dbg;              // experiment switch (AO_DBG): 1 = skip the row march, 2 = skip staging, 4 = skip image formation
+#ifdef AO_PROFILE_SWITCHES
+    int dbg;              // profiling builds only (AO_DBG): 1 = skip the row march, 2 = skip staging, 4 = skip image formation
+#endif
 };
+
+// Component-timing switches exist in profiling builds only (AO_BUILD_PROFILE=1); a normal build compiles them out.
+#ifdef AO_PROFILE_SWITCHES
+#define AO_DBG_ON(args, bit) (((args).dbg & (bit)) != 0)
+#else
+#define AO_DBG_ON(args, bit) false
+#endif
 
 // Per active layer, built in the prologue (dynamic shared memory).
 struct __align__(16) LayerT {
@@ -257,7 +266,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             if (i == 0) R0[stage * kKS + s] = (int)r;
         }
         __syncwarp();
-        if (A.dbg & 2) return;
+        if (AO_DBG_ON(A, 2)) return;
         if (lane == 0) mbar_expect_tx(bar, (uint32_t)(rt * wt) * 4u);
         __syncwarp();
         const int first = (cw + wt <= Sn) ? wt : Sn - cw;                     // floats before the periodic wrap
@@ -278,7 +287,6 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
 
     const uint32_t tiles_s = smem_u32(tiles), w_s = smem_u32(Wt);
     const uint32_t pb = (uint32_t)pitch * 4u, tile_bytes = (uint32_t)tile_floats * 4u;
-    const int dbg = A.dbg;
     int stage = 0;
     uint32_t par = 0;                          // stage and parity of layer a
     // Refill lag: at iteration a the producer refills the stage of layer a - lag with layer a - lag + ns.  With
@@ -289,7 +297,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
     for (int a = 0; a < nact; ++a) {
         // the producer role rotates over the warps: a fixed producer warp would lag by its issue + table time
         // every layer and pace the whole CTA
-        if (warp == (a & (NT / 32 - 1)) && a >= lag && a - lag + ns < nact && !(A.dbg & 8)) {
+        if (warp == (a & (NT / 32 - 1)) && a >= lag && a - lag + ns < nact && !AO_DBG_ON(A, 8)) {
             const int l = a - lag, m = l / ns;
             mbar_wait(&S.empty_bar[l - m * ns], (uint32_t)(m & 1));
             issue(l + ns, l - m * ns);
@@ -300,7 +308,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         const uint32_t tile_s = tiles_s + (uint32_t)stage * tile_bytes;
         const u64 colA = (u64)(unsigned)tid * du64, colB = colA + (u64)NT * du64;
         const u64 colW = (u64)(unsigned)(tid & ~31) * du64;
-        if (!(A.dbg & 2)) mbar_wait(&S.full_bar[stage], par);
+        if (!AO_DBG_ON(A, 2)) mbar_wait(&S.full_bar[stage], par);
         const int ro0 = R0[stage * kKS], ro1 = R0[stage * kKS + 1];
         u64 ref;
         {
@@ -311,7 +319,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             if (REFSUM) { refsum[0] += (double)r0f; refsum[1] += (double)r1f; }
         }
         const float k32 = 2.3283064365386963e-10f;             // 2^-32
-        if (!(dbg & 1)) {
+        if (!AO_DBG_ON(A, 1)) {
             {
                 const u64 U0 = uf0 + colA, U1 = uf0 + colB;
                 const u64 fx = pack2(__uint2float_rn((unsigned)U0) * k32, __uint2float_rn((unsigned)U1) * k32);

@@ -34,7 +34,7 @@ inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, 
             if (!(du > 0.0) || du > 8.0) return pl;               // absurd sampling ratio: not this path
             if (du < 0.5 || du > 1.0) pl.anydu = 1;                // outside the three-term march: two-row march
             if (du > du_max) du_max = du;
-            if (lp.S % 4 != 0) return pl;                          // 16-byte aligned rows for the bulk copies
+            if (lp.S % 4 != 0 || ((uintptr_t)lp.screen & 15) != 0) return pl;   // 16-byte aligned rows for the bulk copies
             const double shx = fabs(lp.wx * dt * lp.inv_pitch) * (kKS - 1), shy = fabs(lp.wy * dt * lp.inv_pitch) * (kKS - 1);
             ext_x = std::max(ext_x, (kTileCols - 1) * du + shx);
             ext_y = std::max(ext_y, (kTR - 1) * du + shy);
@@ -54,7 +54,9 @@ inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, 
     const size_t budget = 55 * 1024 + 512;
     pl.ns = 2;
     while (pl.ns < kT2MaxStages && (pl.ns + 1) * stage + sched + 128 + 256 <= budget) ++pl.ns;
+#ifdef AO_PROFILE_SWITCHES      // profiling builds only: override the stage count
     if (const char* ev = getenv("AO_FUSED_STAGES")) { const int v = atoi(ev); if (v >= 2 && v <= kT2MaxStages) pl.ns = v; }
+#endif
     size_t region = pl.ns * stage;
     if (region < min_bytes) region = (min_bytes + 15) & ~(size_t)15;
     pl.smem = region + sched + 128;
@@ -67,7 +69,6 @@ inline Trace2Args make_trace2_args(const ao_geometry* g, const Tile2Plan& pl, in
     Trace2Args t;
     t.layers = g->d_layers; t.n_layers = (int)g->layers.size(); t.srcs = g->d_sources;
     t.step0 = (long long)step0; t.dt = dt; t.pitch = pl.pitch; t.rows = pl.rows; t.ns = pl.ns;
-    t.dbg = 0;
 #ifdef AO_PROFILE_SWITCHES      // profiling builds only (AO_BUILD_PROFILE=1): switch parts of the kernel off, results are wrong
     { const char* ev = getenv("AO_DBG"); t.dbg = ev ? atoi(ev) : 0; }
 #endif
