@@ -240,6 +240,13 @@ int ao_forward_host(ao_geometry* g, const float* const* screens_host, int64_t st
                     double dt_s, const ao_noise* noise, float* const* slopes_host,
                     float* psf_host, void* cuda_stream);
 
+/* ao_probe_fp32 -- measurement aid for the roofline line of bench.py ("the builder must also
+ * measure an FMA-chain micro-benchmark"): runs an FMA-chain micro-kernel (8 independent chains per thread, 8 CTAs of
+ * 256 threads per SM) five times on the legacy default stream, times it with CUDA events and returns the best FP32
+ * rate in TFLOP/s.  packed = 0: scalar FFMA; packed != 0: FFMA2 (fma.rn.f32x2).  Synchronous.
+ * Errors: AO_ERR_INVALID_ARG (NULL), AO_ERR_CUDA. */
+int ao_probe_fp32(ao_geometry* g, int packed, double* tflops_out);
+
 /* Number of kernel launches issued by this handle since creation (all ao_* calls). */
 int64_t ao_launch_count(const ao_geometry* g);
 
