@@ -49,6 +49,9 @@ def lib():
         L.aoref_cdft2.argtypes = [_dp, _dp, C.c_int, C.c_int, C.c_int, C.c_int, _dp, _dp]
         L.aoref_sh_images.argtypes = [_dp, _fp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                       C.c_double, _dp, _u8p]
+        L.aoref_sh_images_elong.argtypes = [_dp, _fp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double,
+                                            C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                            C.c_int, _dp, _dp, _dp, _u8p]
         L.aoref_centroids.argtypes = [_dp, C.c_int, C.c_int, _u8p, _dp, _dp]
         L.aoref_psf.argtypes = [_dp, _fp, C.c_int, C.c_int, C.c_int, _dp]
         L.aoref_philox4x32_10.argtypes = [_u32p, _u32p, _u32p]
@@ -119,6 +122,23 @@ def sh_images(phase: np.ndarray, amp: np.ndarray, n_sub, n, M, beta, P, min_illu
     return img, valid
 
 
+# ------------------------------------------------------------------------------- O9
+def sh_images_elong(phase, amp, n_sub, n, M, beta, P, min_illum, d, lambda_m, H, launch_xy, z, rho):
+    """LGS images with an extended sodium layer (aoref_sh_images_elong): z, rho = altitudes [m] and weights of the
+    scatterers, launch_xy = launch point [m].  -> images [n_sub^2][P][P] fp64, valid [n_sub^2] uint8."""
+    phase = np.ascontiguousarray(phase, dtype=np.float64)
+    amp = np.ascontiguousarray(amp, dtype=np.float32)
+    z = np.ascontiguousarray(z, dtype=np.float64); rho = np.ascontiguousarray(rho, dtype=np.float64)
+    assert phase.shape == (n_sub * n, n_sub * n) and amp.shape == phase.shape and z.shape == rho.shape
+    img = np.empty((n_sub * n_sub, P, P), dtype=np.float64)
+    valid = np.empty(n_sub * n_sub, dtype=np.uint8)
+    _check(lib().aoref_sh_images_elong(_d(phase), amp.ctypes.data_as(_fp), n_sub, n, M, beta, P, float(min_illum),
+                                       float(d), float(lambda_m), float(H), float(launch_xy[0]), float(launch_xy[1]),
+                                       int(z.size), _d(z), _d(rho), _d(img), valid.ctypes.data_as(_u8p)),
+           "sh_images_elong")
+    return img, valid
+
+
 # ------------------------------------------------------------------------------- O6
 def centroids(images: np.ndarray, valid=None):
     """images [n][P][P] -> slopes [2][n] (x block then y block), detector pixels."""
@@ -144,6 +164,35 @@ def psf(phase: np.ndarray, amp: np.ndarray, M: int, into: np.ndarray | None = No
         acc = 0
     _check(lib().aoref_psf(_d(phase), amp.ctypes.data_as(_fp), N, M, acc, _d(into)), "psf")
     return into
+
+
+# ------------------------------------------------------------------------------- O8
+def psf_poly(phase: np.ndarray, amp: np.ndarray, M: int, lambda_s: float, lambdas, weights,
+             into: np.ndarray | None = None) -> np.ndarray:
+    """Polychromatic science PSF on the detector pixel grid of the direction's own wavelength lambda_s (PAPER.md:86
+    section 2.8: "The user select the wavelength at which the PSF is computed and the pixelscale ... The user may desire
+    more wavelengths, considering a bandwidth"; DESIGN.md section 3 reading O8).  phase is in radians at lambda_s.
+    With s_j = lambda_s / lambda_j (the same optical path is s_j phi radians at lambda_j, and the diffraction pattern
+    is 1/s_j times wider on pixels of fixed angular size lambda_s / (M d_p)):
+        E_j = A exp(i s_j phi);   Et_j[k][m] = sum_ab E_j[a][b] exp(-2 pi i s_j ((k - M/2) a + (m - M/2) b) / M)
+        PSF = sum_j w_j s_j^2 |Et_j|^2 / (M^2 sum A^2)
+    (s_j^2: flux per pixel of fixed solid angle; every wavelength integrates to w_j over the whole plane).  One
+    wavelength equal to lambda_s with weight 1 is aoref_psf.  The definition written out: the scaled DFT is two dense
+    FP64 matrix products F E F^T with F[k][a] = exp(-2 pi i s_j (k - M/2) a / M) (numpy matmul is the library step)."""
+    ph = np.asarray(phase, dtype=np.float64)
+    A = np.asarray(amp, dtype=np.float64)
+    N = ph.shape[0]
+    out = np.zeros((M, M), dtype=np.float64) if into is None else into
+    sumA2 = float((A * A).sum())
+    kap = np.arange(M, dtype=np.float64) - M / 2.0
+    a = np.arange(N, dtype=np.float64)
+    for lam, w in zip(lambdas, weights):
+        s = float(lambda_s) / float(lam)
+        E = A * np.exp(1j * s * ph)
+        F = np.exp(-2j * np.pi * s * np.outer(kap, a) / M)               # [M][N]
+        Et = (F @ E) @ F.T
+        out += float(w) * s * s * (Et.real ** 2 + Et.imag ** 2) / (M * M * sumA2)
+    return out
 
 
 # ------------------------------------------------------------------------------- O5
@@ -211,6 +260,9 @@ def forward(cfg, step0: int = 0, n_steps: int = 1, *, want_phase=True, want_wfs=
       psf[s]     : [M][M] long-exposure SUM over the steps (science sources)
     cfg.phase_maps[s] (optional, [N_s][N_s] radians at the source's wavelength) is added to the traced phase of
     source s at every step (section 2.3) before the WFS and the PSF see it.
+    cfg.sodium (optional, inputs.Sodium): the sensors of that WFS see an extended beacon (reading O9); time step
+    step0 + k uses profile row (step0 + k) mod n_t.  cfg.psf_band (optional, (wavelengths, weights)): the science PSF
+    is the polychromatic sum of reading O8 on the pixel grid of each direction's own wavelength.
     Plain loop over steps and sources; every number comes from ao_oracle.c (the map sum is one numpy add).
     """
     res = {"phase": {}, "images": {}, "noisy": {}, "counts": {}, "slopes": {}, "valid": {}, "psf": {}}
@@ -237,7 +289,15 @@ def forward(cfg, step0: int = 0, n_steps: int = 1, *, want_phase=True, want_wfs=
                 ph_list.append(ph)
             if w >= 0 and want_wfs:
                 W = cfg.wfs[w]
-                img, valid = sh_images(ph, W.amp, W.n_sub, W.n_samp, W.fft, W.bin, W.n_pix, W.min_illum)
+                na = getattr(cfg, "sodium", None)
+                if na is not None and na.wfs_index == w:
+                    rho = np.asarray(na.rho, dtype=np.float64)
+                    img, valid = sh_images_elong(ph, W.amp, W.n_sub, W.n_samp, W.fft, W.bin, W.n_pix, W.min_illum,
+                                                 d, src.lambda_m, src.altitude_m,
+                                                 na.launch_xy_m[cfg.sources_of_wfs(w).index(s)], na.z_m,
+                                                 rho[(step0 + k) % rho.shape[0]])
+                else:
+                    img, valid = sh_images(ph, W.amp, W.n_sub, W.n_samp, W.fft, W.bin, W.n_pix, W.min_illum)
                 res["valid"][w] = valid
                 im_list.append(img)
                 use = img
@@ -248,7 +308,10 @@ def forward(cfg, step0: int = 0, n_steps: int = 1, *, want_phase=True, want_wfs=
                     use = nz
                 sl_list.append(centroids(use, valid))
             if w < 0 and want_psf and cfg.psf_fft:
-                if acc is None:
+                band = getattr(cfg, "psf_band", None)
+                if band is not None:
+                    acc = psf_poly(ph, cfg.pupil.amp, cfg.psf_fft, src.lambda_m, band[0], band[1], into=acc)
+                elif acc is None:
                     acc = psf(ph, cfg.pupil.amp, cfg.psf_fft)
                 else:
                     psf(ph, cfg.pupil.amp, cfg.psf_fft, into=acc)

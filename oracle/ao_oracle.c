@@ -19,7 +19,9 @@
  * (tests/golden/), Parseval, flat->zero slopes, piston invariance, linear-screen
  * bilinear exactness, integer/half-pixel shifts, cone scaling, periodicity,
  * cuRAND's host Philox4_32_10 generator, scipy.stats.poisson.ppf (mu up to 1e4), Poisson/Gauss statistics.
- * No function here is "parity unpinned".
+ * O8 (polychromatic PSF, oracle/__init__.py psf_poly) and O9 (LGS elongation, aoref_sh_images_elong) are pinned by
+ * closed forms too (one wavelength = aoref_psf, the 2M crop identity, Dirichlet products; delta profile = aoref_sh_images,
+ * whole-pixel shifts along the launch-to-subaperture direction, energy).  No function here is "parity unpinned".
  *
  * Layout: all arrays row-major [y][x], x fastest.
  */
@@ -304,6 +306,85 @@ int aoref_sh_images(const double* phase, const float* amp, int n_sub, int n, int
                     }
                 img[r * P + c] = s;
             }
+        free(e_re); free(e_im); free(o_re); free(o_im);
+    }
+    return err;
+}
+
+/* ------------------------------------------------------------------------------------
+ * O9  Shack-Hartmann images of a laser guide star with an extended sodium layer (section 2.7: "It's possible
+ * to consider at this level the sodium layer temporal evolution"; DESIGN.md section 3
+ * reading O9).  The paper gives no formula; the reading is plain geometry.
+ *
+ * The beacon is a column of n_z scatterers at altitudes z_i with weights rho_i (the sodium profile at this time step,
+ * caller-supplied), on the line from the launch point L = (launch_x, launch_y) [m, pupil plane] to the focus point at
+ * altitude H.  Seen from the subaperture centred at c, the scatterer at z_i is displaced from the focus point by the angle
+ *     delta_i = (c - L) (1/H - 1/z_i)                                (small angles; zero for z_i = H)
+ * which is a tilt of  alpha_i = 2 pi delta_i d / lambda  radians per sample across the subaperture (d = sample pitch),
+ * i.e. a shift of the spot by delta_i M d / lambda FFT pixels along c - L.  The detector integrates incoherently:
+ *     I = sum_i rho_i |DFT_M( A exp(i (phi + alpha_ix b + alpha_iy a)) )|^2 / (M^2 n^2),   then binned as in O4.
+ * Subaperture centre: x_c = ((q n + (n-1)/2) - (N-1)/2) d, y_c with p (O1 grid).  Validity as in aoref_sh_images.
+ * n_z = 1 with z_0 = H reproduces aoref_sh_images.
+ */
+int aoref_sh_images_elong(const double* phase, const float* amp, int n_sub, int n, int M, int beta, int P,
+                          double min_illum, double d, double lambda_m, double H, double launch_x, double launch_y,
+                          int n_z, const double* z, const double* rho, double* images, uint8_t* valid)
+{
+    if (!phase || !amp || !images || !valid || !z || !rho || n_z <= 0 || n_sub <= 0 || n <= 0 || M < n || beta <= 0 ||
+        P <= 0 || beta * P > M || ((M - beta * P) & 1) || M > 64)
+        return AOREF_ERR_ARG;
+    const int N = n_sub * n, nsa = n_sub * n_sub;
+    const int k0 = (M - beta * P) / 2;
+    int err = 0;
+    #pragma omp parallel for schedule(dynamic, 4)
+    for (int sa = 0; sa < nsa; ++sa) {
+        const int p = sa / n_sub, q = sa % n_sub;
+        double* img = images + (size_t)sa * P * P;
+        for (int i = 0; i < P * P; ++i) img[i] = 0.0;
+        double illum = 0.0;
+        for (int a = 0; a < n; ++a)
+            for (int b = 0; b < n; ++b) {
+                const double A = amp[(size_t)(p * n + a) * N + q * n + b];
+                illum += A * A;
+            }
+        illum /= (double)n * n;
+        valid[sa] = (uint8_t)(illum >= min_illum);
+        if (!valid[sa]) continue;
+        double* e_re = (double*)malloc(sizeof(double) * n * n);
+        double* e_im = (double*)malloc(sizeof(double) * n * n);
+        double* o_re = (double*)malloc(sizeof(double) * (size_t)M * M);
+        double* o_im = (double*)malloc(sizeof(double) * (size_t)M * M);
+        if (!e_re || !e_im || !o_re || !o_im) {
+            free(e_re); free(e_im); free(o_re); free(o_im);
+            #pragma omp atomic write
+            err = AOREF_ERR_ALLOC;
+            continue;
+        }
+        const double xc = (((double)q * n + (double)(n - 1) / 2.0) - (double)(N - 1) / 2.0) * d;
+        const double yc = (((double)p * n + (double)(n - 1) / 2.0) - (double)(N - 1) / 2.0) * d;
+        const double norm = 1.0 / ((double)M * M * (double)n * n);
+        for (int iz = 0; iz < n_z; ++iz) {
+            const double g = 2.0 * M_PI * (1.0 / H - 1.0 / z[iz]) * d / lambda_m;       /* rad per sample per metre of baseline */
+            const double ax = g * (xc - launch_x), ay = g * (yc - launch_y);
+            for (int a = 0; a < n; ++a)
+                for (int b = 0; b < n; ++b) {
+                    const size_t gi = (size_t)(p * n + a) * N + q * n + b;
+                    const double A = amp[gi], ph = phase[gi] + ax * (double)b + ay * (double)a;
+                    e_re[a * n + b] = A * cos(ph);
+                    e_im[a * n + b] = A * sin(ph);
+                }
+            aoref_cdft2(e_re, e_im, n, M, 1, 0, o_re, o_im);
+            for (int r = 0; r < P; ++r)
+                for (int c = 0; c < P; ++c) {
+                    double s = 0.0;
+                    for (int k = k0 + beta * r; k < k0 + beta * r + beta; ++k)
+                        for (int m = k0 + beta * c; m < k0 + beta * c + beta; ++m) {
+                            const double xr = o_re[(size_t)k * M + m], xi = o_im[(size_t)k * M + m];
+                            s += (xr * xr + xi * xi) * norm;
+                        }
+                    img[r * P + c] += rho[iz] * s;
+                }
+        }
         free(e_re); free(e_im); free(o_re); free(o_im);
     }
     return err;

@@ -79,6 +79,17 @@ class Noise:
 
 
 @dataclass
+class Sodium:
+    """Extended sodium layer seen by the LGS sensors of one WFS (reading O9): scatterer altitudes z [n_z],
+    weights rho [n_t][n_z] (row (step mod n_t) is the profile of a time step: the temporal evolution), and the launch
+    point of every source of that WFS [n_src_w][2] in metres in the pupil plane."""
+    wfs_index: int
+    z_m: np.ndarray
+    rho: np.ndarray
+    launch_xy_m: np.ndarray
+
+
+@dataclass
 class Config:
     name: str
     pupil: Pupil
@@ -96,6 +107,8 @@ class Config:
     notes: dict = field(default_factory=dict)
     # static additive phase maps: source index -> [N_s][N_s] float32 radians at the source's wavelength
     phase_maps: dict = field(default_factory=dict)
+    sodium: Optional[Sodium] = None          # NEXT-3: LGS spot elongation (None: point beacon at the source altitude)
+    psf_band: Optional[tuple] = None         # NEXT-4: (wavelengths_m [n], weights [n]) of the polychromatic science PSF
 
     # ---- derived shapes (no arithmetic of the method; only sizes) ----
     def grid_n(self, s: int) -> int:
@@ -321,6 +334,28 @@ def make_config(index: int, *, n_sub: Optional[int] = None, screen_n: Optional[i
     if with_screens:
         fill_screens(cfg, device=device, keep_on_device=keep_on_device)
     return cfg
+
+
+def sodium_profile(cfg: Config, wfs_index: int = 0, n_z: int = 5, n_t: int = 8, mean_m: float = 90e3,
+                   fwhm_m: float = 10e3, launch: str = "centre", seed: Optional[int] = None) -> Sodium:
+    """Synthetic sodium layer (the paper's profile is not given): n_z equally spaced scatterers over +-1.25 FWHM
+    around a mean altitude that drifts by up to +-500 m over the n_t time samples, Gaussian weights plus a seeded
+    sporadic component on one slab, each row normalised to 1.  launch = "centre" (behind the secondary mirror) or
+    "side" (at the pupil edge, on the azimuth of each beacon).  Input data only: no arithmetic of the method."""
+    rng = np.random.default_rng(np.random.PCG64((cfg.seed if seed is None else seed) + 4099))
+    sigma = fwhm_m / 2.3548200450309493
+    z = mean_m + np.linspace(-1.25, 1.25, n_z) * fwhm_m
+    drift = 500.0 * np.sin(2.0 * math.pi * np.arange(n_t) / max(n_t, 1) + rng.uniform(0, 2 * math.pi))
+    rho = np.exp(-0.5 * ((z[None, :] - (mean_m + drift[:, None])) / sigma) ** 2)
+    rho[:, rng.integers(0, n_z)] *= 1.0 + 0.5 * rng.uniform(0.0, 1.0, n_t)
+    rho /= rho.sum(axis=1, keepdims=True)
+    srcs = cfg.sources_of_wfs(wfs_index)
+    xy = np.zeros((len(srcs), 2))
+    if launch == "side":
+        for i, s in enumerate(srcs):
+            az = math.atan2(cfg.sources[s].theta_y_rad, cfg.sources[s].theta_x_rad)
+            xy[i] = (cfg.pupil.r_out_m * math.cos(az), cfg.pupil.r_out_m * math.sin(az))
+    return Sodium(wfs_index, z, rho, xy)
 
 
 def linear_screen(n: int, c0: float, c_row: float, c_col: float) -> np.ndarray:

@@ -758,3 +758,174 @@ def test_big_fft_sensor_image_closed_form_flat_and_integer_tilt():
     ph2 = np.zeros((2 * n, 2 * n)); ph2[:n, n:] = tilt.T
     img2, v2 = oracle.sh_images(ph2, np.ones((2 * n, 2 * n), np.float32), 2, n, M, beta, P, 0.0)
     assert np.abs(img2[1] - np.outer(px, prof)).max() < 1e-13 and np.abs(img2[0] - np.outer(prof, prof)).max() < 1e-13
+
+
+# ----------------------------------------------------------------------------- NEXT-4: polychromatic PSF (reading O8)
+def _dirichlet_scaled(N, M, s):
+    """|sum_{a<N} exp(-2 pi i s kappa a / M)|^2 = sin^2(N psi/2)/sin^2(psi/2), psi = 2 pi s kappa/M, kappa = k - M/2."""
+    psi = 2.0 * np.pi * s * (np.arange(M) - M / 2.0) / M
+    sn = np.sin(psi / 2.0)
+    with np.errstate(all="ignore"):
+        return np.where(np.abs(sn) < 1e-13, float(N * N), np.sin(N * psi / 2.0) ** 2 / sn ** 2)
+
+
+def test_psf_poly_one_wavelength_is_the_monochromatic_psf():
+    N, M = 24, 64
+    amp = inputs.annulus_mask(N, 0.04, N * 0.02, 0.12)
+    ph = RNG.standard_normal((N, N))
+    mono = oracle.psf(ph, amp, M)
+    poly = oracle.psf_poly(ph, amp, M, 2.2e-6, [2.2e-6], [1.0])
+    assert np.abs(poly - mono).max() < 1e-13
+    acc = oracle.psf_poly(ph, amp, M, 2.2e-6, [2.2e-6], [0.25], into=mono.copy())       # accumulates, weights scale
+    assert np.abs(acc - 1.25 * mono).max() < 1e-13
+
+
+def test_psf_poly_flat_square_pupil_is_the_weighted_sum_of_scaled_dirichlet_products():
+    """Two wavelengths on a flat square pupil: each contributes w_j s_j^2 D(s_j kappa_k) D(s_j kappa_m) / (M^2 N^2), a
+    diffraction pattern 1/s_j times wider on the fixed pixel grid (the lambda-dependent pixel scale), peak w_j s_j^2 N^2/M^2."""
+    N, M, lam_s = 10, 48, 2.0e-6
+    lams, wts = [1.6e-6, 2.5e-6], [0.7, 0.3]
+    p = oracle.psf_poly(np.zeros((N, N)), np.ones((N, N), np.float32), M, lam_s, lams, wts)
+    want = np.zeros((M, M))
+    for lam, w in zip(lams, wts):
+        s = lam_s / lam
+        D = _dirichlet_scaled(N, M, s)
+        want += w * s * s * np.outer(D, D) / (M * M * N * N)
+    assert np.abs(p - want).max() < 1e-13
+    assert abs(p[M // 2, M // 2] - sum(w * (lam_s / l) ** 2 for l, w in zip(lams, wts)) * N * N / M ** 2) < 1e-14
+    # first zero of the longer wavelength is further out: kappa = M / (N s)
+    s_long = lam_s / 2.5e-6
+    only = oracle.psf_poly(np.zeros((N, N)), np.ones((N, N), np.float32), M, lam_s, [2.5e-6], [1.0])
+    assert abs(M / (N * s_long) - 6.0) < 1e-12 and only[M // 2, M // 2 + 6] < 1e-28 < only[M // 2, M // 2 + 5]
+
+
+def test_psf_poly_twice_the_wavelength_is_the_central_crop_of_the_2M_transform():
+    """s = 1/2: exp(-2 pi i kappa a / (2M)) is the pixel-centred DFT of size 2M, so the PSF at lambda = 2 lambda_s on
+    M pixels equals the central M x M crop of aoref_psf at size 2M of the phase scaled by 1/2 (normalisation included:
+    s^2 / M^2 = 1 / (2M)^2).  An independent route through the pinned C transform."""
+    N, M = 20, 32
+    amp = inputs.annulus_mask(N, 0.04, N * 0.02, 0.1)
+    ph = RNG.standard_normal((N, N)) * 2.0
+    poly = oracle.psf_poly(ph, amp, M, 1.0e-6, [2.0e-6], [1.0])
+    big = oracle.psf(0.5 * ph, amp, 2 * M)
+    assert np.abs(poly - big[M // 2:M // 2 + M, M // 2:M // 2 + M]).max() < 1e-13
+
+
+def test_psf_poly_tilt_is_achromatic_in_angle_and_energy_stays_in_the_field():
+    """A tilt of optical path moves every wavelength to the same detector pixel (phase scales with s, so does the
+    frequency axis); and a compact PSF keeps sum = sum of weights to the part that leaves the field."""
+    N, M, lam_s = 16, 64, 1.0e-6
+    t = 7
+    ph = np.tile(2 * np.pi * t / M * np.arange(N), (N, 1))                     # radians at lambda_s
+    for lam in (0.8e-6, 1.0e-6, 1.7e-6):
+        p = oracle.psf_poly(ph, np.ones((N, N), np.float32), M, lam_s, [lam], [1.0])
+        assert np.unravel_index(np.argmax(p), p.shape) == (M // 2, M // 2 + t)
+    ph = RNG.standard_normal((N, N)) * 0.3
+    p = oracle.psf_poly(ph, np.ones((N, N), np.float32), 8 * N, lam_s, [1.5e-6, 2.0e-6], [0.6, 0.4])
+    assert 0.93 < p.sum() <= 1.0 + 1e-12                                        # wider than one period never happens for s < 1
+    res = oracle.forward(_poly_cfg(), 0, 2, want_wfs=False)
+    assert set(res["psf"]) == {0}
+
+
+def _poly_cfg():
+    cfg = inputs.make_config(3, n_sub=4, screen_n=128, n_steps=2, n_layers=2)
+    cfg.sources = [cfg.sources[-1]]; cfg.sources[0].wfs_index = -1
+    cfg.wfs = []
+    cfg.psf_band = ([2.0e-6, 2.2e-6, 2.4e-6], [0.3, 0.4, 0.3])
+    return cfg
+
+
+def test_forward_uses_the_band_for_every_step_of_the_long_exposure():
+    cfg = _poly_cfg()
+    res = oracle.forward(cfg, 3, 2, want_wfs=False)
+    want = np.zeros((cfg.psf_fft, cfg.psf_fft))
+    for k in range(2):
+        oracle.psf_poly(res["phase"][0][k], cfg.pupil.amp, cfg.psf_fft, cfg.sources[0].lambda_m, *cfg.psf_band, into=want)
+    assert np.array_equal(res["psf"][0], want)
+    cfg.psf_band = None
+    mono = oracle.forward(cfg, 3, 2, want_wfs=False)["psf"][0]
+    assert np.abs(mono - want).max() > 1e-6                                     # the band does change the image
+
+
+# ----------------------------------------------------------------------------- NEXT-3: LGS elongation (reading O9)
+def _elong(phase, n_sub, n, M, beta, P, z, rho, launch=(0.0, 0.0), d=0.03, lam=589e-9, H=90e3, amp=None):
+    amp = np.ones((n_sub * n, n_sub * n), np.float32) if amp is None else amp
+    return oracle.sh_images_elong(phase, amp, n_sub, n, M, beta, P, 0.5, d, lam, H, launch, z, rho)
+
+
+def test_elongation_delta_profile_at_the_focus_altitude_changes_nothing():
+    n_sub, n, M, beta, P = 4, 8, 16, 2, 8
+    ph = RNG.standard_normal((n_sub * n, n_sub * n))
+    amp = inputs.annulus_mask(n_sub * n, 0.03, n_sub * n * 0.015, 0.1)
+    ref, v0 = oracle.sh_images(ph, amp, n_sub, n, M, beta, P, 0.5)
+    img, v1 = _elong(ph, n_sub, n, M, beta, P, [90e3], [1.0], launch=(3.0, -2.0), amp=amp)
+    assert np.array_equal(v0, v1) and np.array_equal(img, ref)
+    # several scatterers, all at H: still the point-beacon image (weights sum to 1)
+    img2, _ = _elong(ph, n_sub, n, M, beta, P, [90e3] * 3, [0.2, 0.5, 0.3], launch=(3.0, -2.0), amp=amp)
+    assert np.abs(img2 - ref).max() < 1e-15
+
+
+def test_elongation_is_a_whole_pixel_shift_along_the_launch_to_subaperture_direction():
+    """One scatterer above the focus altitude, chosen so that the spot of the subaperture one pitch to the right of the
+    launch point moves by exactly one detector pixel: delta = (c - L)(1/H - 1/z), shift = delta M d / lambda FFT pixels.
+    The shift grows linearly with the baseline, points away from the launch point for z > H (towards it for z < H), and
+    is along y for subapertures above / below the launch point."""
+    n_sub, n, M, beta, P, d, lam, H = 5, 8, 16, 2, 8, 0.05, 589e-9, 90e3
+    N = n_sub * n
+    ph = np.zeros((N, N))
+    base, _ = oracle.sh_images(ph, np.ones((N, N), np.float32), n_sub, n, M, beta, P, 0.5)
+    pitch = n * d                                                  # distance between subaperture centres
+    # launch at the centre of subaperture (2, 2) = the grid centre; one-pixel shift (beta FFT pixels) per pitch
+    inv = 1.0 / H - beta * lam / (M * d * pitch)                   # 1/z with (1/H - 1/z) pitch M d / lambda = beta
+    z = 1.0 / inv
+    assert z > H
+    img, _ = _elong(ph, n_sub, n, M, beta, P, [z], [1.0], d=d, lam=lam, H=H)
+    sub = lambda p, q: img[p * n_sub + q]
+    assert np.abs(sub(2, 2) - base[0]).max() < 1e-14                                   # on the launch axis: no shift
+    assert np.abs(sub(2, 3) - np.roll(base[0], 1, axis=1)).max() < 1e-13               # +x neighbour: one pixel to +x
+    assert np.abs(sub(2, 4) - np.roll(base[0], 2, axis=1)).max() < 1e-13               # twice the baseline: two pixels
+    assert np.abs(sub(2, 1) - np.roll(base[0], -1, axis=1)).max() < 1e-13              # -x neighbour: to -x
+    assert np.abs(sub(3, 2) - np.roll(base[0], 1, axis=0)).max() < 1e-13               # +y neighbour: rows
+    assert np.abs(sub(0, 4) - np.roll(np.roll(base[0], -2, axis=0), 2, axis=1)).max() < 1e-13
+    # below the focus altitude the spot moves towards the launch point
+    z_lo = 1.0 / (1.0 / H + beta * lam / (M * d * pitch))
+    lo, _ = _elong(ph, n_sub, n, M, beta, P, [z_lo], [1.0], d=d, lam=lam, H=H)
+    assert np.abs(lo[2 * n_sub + 3] - np.roll(base[0], -1, axis=1)).max() < 1e-13
+    # a launch point moved by one pitch moves the pattern with it
+    off, _ = _elong(ph, n_sub, n, M, beta, P, [z], [1.0], launch=(pitch, 0.0), d=d, lam=lam, H=H)
+    assert np.abs(off[2 * n_sub + 3] - base[0]).max() < 1e-13 and np.abs(off[2 * n_sub + 2] - np.roll(base[0], -1, axis=1)).max() < 1e-13
+
+
+def test_elongated_image_is_the_profile_weighted_sum_and_conserves_energy():
+    n_sub, n, M, beta, P, d, lam, H = 5, 8, 16, 2, 8, 0.05, 589e-9, 90e3
+    N = n_sub * n
+    ph = RNG.standard_normal((N, N)) * 0.7
+    amp = inputs.annulus_mask(N, d, N * d / 2, 0.3)
+    z = np.array([84e3, 88e3, 90e3, 93e3, 97e3]); rho = np.array([0.1, 0.25, 0.3, 0.2, 0.15])
+    img, valid = _elong(ph, n_sub, n, M, beta, P, z, rho, launch=(-0.4, 0.9), d=d, lam=lam, H=H, amp=amp)
+    parts = [_elong(ph, n_sub, n, M, beta, P, [zi], [1.0], launch=(-0.4, 0.9), d=d, lam=lam, H=H, amp=amp)[0] for zi in z]
+    assert np.abs(img - sum(r * p for r, p in zip(rho, parts))).max() < 1e-15         # incoherent sum over the column
+    point, _ = oracle.sh_images(ph, amp, n_sub, n, M, beta, P, 0.5)
+    assert np.abs(img.sum(axis=(1, 2)) - point.sum(axis=(1, 2))).max() < 1e-13         # full window: Parseval per scatterer
+    # the spot is longer along the baseline: second moment along c - L grows, across it it does not shrink the energy
+    far = 0 * n_sub + 4 if valid[4] else int(np.flatnonzero(valid)[0])
+    assert img[far].max() < point[far].max()
+
+
+def test_forward_picks_the_profile_of_the_absolute_step():
+    cfg = inputs.make_config(2, n_sub=6, screen_n=128, n_steps=2, n_layers=2)
+    cfg.sources = cfg.sources[:2]
+    cfg.sodium = inputs.sodium_profile(cfg, n_z=3, n_t=4, launch="side")
+    assert cfg.sodium.rho.shape == (4, 3) and np.allclose(cfg.sodium.rho.sum(axis=1), 1.0)
+    res = oracle.forward(cfg, 6, 2)
+    W = cfg.wfs[0]
+    for s in (0, 1):
+        for k in (0, 1):
+            img, _ = oracle.sh_images_elong(res["phase"][s][k], W.amp, W.n_sub, W.n_samp, W.fft, W.bin, W.n_pix, W.min_illum,
+                                            cfg.grid_pitch(s), cfg.sources[s].lambda_m, cfg.sources[s].altitude_m,
+                                            cfg.sodium.launch_xy_m[s], cfg.sodium.z_m, cfg.sodium.rho[(6 + k) % 4])
+            assert np.array_equal(res["images"][s][k], img)
+            other, _ = oracle.sh_images_elong(res["phase"][s][k], W.amp, W.n_sub, W.n_samp, W.fft, W.bin, W.n_pix, W.min_illum,
+                                              cfg.grid_pitch(s), cfg.sources[s].lambda_m, cfg.sources[s].altitude_m,
+                                              cfg.sodium.launch_xy_m[s], cfg.sodium.z_m, cfg.sodium.rho[k % 4])
+            assert not np.array_equal(other, img)
