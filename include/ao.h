@@ -177,6 +177,22 @@ int ao_centroids(ao_geometry* g, int wfs_index, const float* images_dev, int n_i
 int ao_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, double dt_s,
            float* psf_dev, int accumulate, void* cuda_stream);
 
+/* ao_set_psf_band / ao_psf_poly -- polychromatic science PSF (section 2.8: "The user select the wavelength at
+ * which the PSF is computed and the pixelscale ... The user may desire more wavelengths, considering a bandwidth"; DESIGN.md
+ * section 3 reading O8).  The detector pixels keep the angular size lambda_s / (M d_p) of the science directions' own
+ * wavelength lambda_s; wavelength lambda_j (s_j = lambda_s / lambda_j) sees the phase s_j phi and a pattern 1/s_j wider:
+ *   PSF_k = sum_j w_j s_j^2 |sum_ab A exp(i s_j phi_k) exp(-2 pi i s_j ((k-M/2) a + (m-M/2) b)/M)|^2 / (M^2 sum A^2),
+ * the scaled DFT being evaluated as a chirp-z transform with FFTs of length L >= M + N_p - 1.  One wavelength equal to
+ * lambda_s with weight 1 is ao_psf.
+ * ao_set_psf_band: lambdas_m_host [n_lambda], weights_host [n_lambda]: HOST arrays, copied; builds the chirp tables in
+ *   FP64 (cudaMalloc; synchronises the device); n_lambda = 0 clears the band.  Needs psf_fft + pupil n - 1 <= 4096 and
+ *   all science directions at one wavelength, else AO_ERR_UNSUPPORTED.  While a band is set, ao_forward and
+ *   ao_forward_host produce the polychromatic PSF; ao_psf stays monochromatic.
+ * ao_psf_poly: same arguments, layout, accumulation and workspace as ao_psf; AO_ERR_INVALID_ARG if no band is set. */
+int ao_set_psf_band(ao_geometry* g, const double* lambdas_m_host, const double* weights_host, int n_lambda);
+int ao_psf_poly(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, double dt_s,
+                float* psf_dev, int accumulate, void* cuda_stream);
+
 /* ao_set_phase_map -- static additive phase map of one source (section 2.3: telescope aberration
  * maps such as M1 scalloping and the NGS-WFS mis-positioning tip/tilt are "summed to the open loop WF"):
  *   phi_s[k, i, j] <- phi_s[k, i, j] + map[i][j]  for every time step k,
@@ -186,6 +202,21 @@ int ao_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, d
  * handle is destroyed.  Synchronises the device (the call updates a table that launches in flight may be reading).
  * Errors: AO_ERR_INVALID_ARG for a bad handle or source index. */
 int ao_set_phase_map(ao_geometry* g, int source, const float* map_dev);
+
+/* ao_set_sodium -- extended sodium layer for the LGS sensors of WFS `wfs_index` (section 2.7: "It's possible to
+ * consider at this level the sodium layer temporal evolution"; DESIGN.md section 3 reading O9).  The beacon of every source of
+ * that WFS becomes a column of n_z scatterers at altitudes z_m[i] with weights rho[t][i]; time step s uses the profile row
+ * t = s mod n_t (the temporal evolution: n_t = 1 is a static profile).  Seen from the subaperture centred at c, scatterer i
+ * is displaced from the focus point (the source altitude H) by the angle (c - L)(1/H - 1/z_i), L = launch_xy_m of the
+ * source: its spot is the point-beacon spot shifted by that angle (a phase ramp over the subaperture, exact on the DFT grid,
+ * periodic in the field of view) and the detector sums the spots with the weights rho (which the caller normalises).
+ *   z_m_host [n_z], rho_host [n_t][n_z], launch_xy_m_host [n_src_w][2] (sources of the WFS in ascending order): HOST
+ *   arrays, copied.  n_z = 0 restores the point beacon.  1 <= n_z <= 64.
+ * Applies to ao_sh_images (both phase_dev paths), ao_forward and ao_forward_host.  Synchronises the device; allocates the
+ * small tables with cudaMalloc (with ao_set_psf_band the only calls after ao_geometry_create that do).
+ * Errors: AO_ERR_INVALID_ARG (bad index, NULL arrays, a source at infinity, z <= 0), AO_ERR_UNSUPPORTED (fft > 64). */
+int ao_set_sodium(ao_geometry* g, int wfs_index, int n_z, const double* z_m_host, const double* rho_host, int n_t,
+                  const double* launch_xy_m_host);
 
 /* ao_modes_to_map -- residual-phase entry (section 2.7: "residual = open loop WF - DM shape", the
  * WFS then measures the residual; section 2.5: the calibration pushes mirror modes through the WFS):

@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "AO_OK", 1: "AO_ERR_INVALID_ARG", 2: "AO_ERR_SHAPE", 3: "AO_E
 # every symbol include/ao.h declares
 EXPORTS = ["ao_geometry_create", "ao_geometry_destroy", "ao_workspace_bytes", "ao_set_workspace",
            "ao_phase_elems_per_step", "ao_phase_offset", "ao_wfs_valid", "ao_trace_layers",
-           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_phase_map", "ao_modes_to_map", "ao_strehl", "ao_strehl_marechal", "ao_forward", "ao_forward_host", "ao_probe_fp32", "ao_launch_count",
+           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_psf_band", "ao_psf_poly", "ao_set_phase_map", "ao_set_sodium", "ao_modes_to_map", "ao_strehl", "ao_strehl_marechal", "ao_forward", "ao_forward_host", "ao_probe_fp32", "ao_launch_count",
            "ao_last_error", "ao_version"]
 
 
@@ -82,7 +82,10 @@ def load_library():
     L.ao_sh_images.argtypes = [vp, i32, vp, i64, i32, dbl, C.POINTER(ao_noise), vp, vp, vp]
     L.ao_centroids.argtypes = [vp, i32, vp, i32, vp, vp]
     L.ao_psf.argtypes = [vp, vp, i64, i32, dbl, vp, i32, vp]
+    L.ao_set_psf_band.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), i32]
+    L.ao_psf_poly.argtypes = [vp, vp, i64, i32, dbl, vp, i32, vp]
     L.ao_set_phase_map.argtypes = [vp, i32, vp]
+    L.ao_set_sodium.argtypes = [vp, i32, i32, C.POINTER(dbl), C.POINTER(dbl), i32, C.POINTER(dbl)]
     L.ao_modes_to_map.argtypes = [vp, vp, i32, i64, vp, C.c_float, vp, vp]
     L.ao_strehl.argtypes = [vp, vp, dbl, vp, vp]
     L.ao_strehl_marechal.argtypes = [vp, vp, i32, vp, vp]
@@ -161,6 +164,10 @@ class Geometry:
         self.set_workspace_steps(workspace_steps)
         for si, m in getattr(cfg, "phase_maps", {}).items():
             self.set_phase_map(si, m)
+        if getattr(cfg, "sodium", None) is not None:
+            self.set_sodium(cfg.sodium)
+        if getattr(cfg, "psf_band", None) is not None:
+            self.set_psf_band(*cfg.psf_band)
 
     # ---- lifetime ----
     def close(self):
@@ -185,6 +192,18 @@ class Geometry:
                             else phase_map, dtype=torch.float32).to(self.device).contiguous()
         self.phase_maps[source] = t                      # borrowed by the library: keep it alive
         _check(self.lib.ao_set_phase_map(self.handle, int(source), _ptr(t)))
+
+    def set_sodium(self, sodium):
+        """ao_set_sodium: extended beacon of one WFS from an inputs.Sodium (None or n_z = 0 clears wfs 0's)."""
+        dp = C.POINTER(C.c_double)
+        if sodium is None:
+            _check(self.lib.ao_set_sodium(self.handle, 0, 0, None, None, 0, None))
+            return
+        z = np.ascontiguousarray(sodium.z_m, dtype=np.float64)
+        rho = np.ascontiguousarray(np.atleast_2d(sodium.rho), dtype=np.float64)
+        xy = np.ascontiguousarray(sodium.launch_xy_m, dtype=np.float64)
+        _check(self.lib.ao_set_sodium(self.handle, int(sodium.wfs_index), int(z.size), z.ctypes.data_as(dp),
+                                      rho.ctypes.data_as(dp), int(rho.shape[0]), xy.ctypes.data_as(dp)))
 
     def modes_to_map(self, modes, coeffs, sign: float, out):
         """ao_modes_to_map: out[i] = sign * sum_m coeffs[m] modes[m][i] (CUDA float32 tensors; out is overwritten)."""
@@ -275,6 +294,25 @@ class Geometry:
         if psf is None:
             psf = torch.zeros((n_sci, M, M), dtype=torch.float32, device=self.device)
         _check(self.lib.ao_psf(self.handle, _ptr(phase), step0, n_steps, dt_s, _ptr(psf), int(accumulate), _stream()))
+        return psf
+
+    def set_psf_band(self, lambdas_m=None, weights=None):
+        """ao_set_psf_band: wavelengths [m] and weights of the polychromatic PSF (None clears the band)."""
+        dp = C.POINTER(C.c_double)
+        if lambdas_m is None:
+            _check(self.lib.ao_set_psf_band(self.handle, None, None, 0))
+            return
+        lam = np.ascontiguousarray(lambdas_m, dtype=np.float64); w = np.ascontiguousarray(weights, dtype=np.float64)
+        assert lam.shape == w.shape
+        _check(self.lib.ao_set_psf_band(self.handle, lam.ctypes.data_as(dp), w.ctypes.data_as(dp), int(lam.size)))
+
+    def psf_poly(self, phase, step0: int, n_steps: int, dt_s: float, psf=None, accumulate=False):
+        """ao_psf_poly: polychromatic long-exposure PSF over the band set with set_psf_band."""
+        import torch
+        M = self.cfg.psf_fft
+        if psf is None:
+            psf = torch.zeros((len(self.cfg.science_sources()), M, M), dtype=torch.float32, device=self.device)
+        _check(self.lib.ao_psf_poly(self.handle, _ptr(phase), step0, n_steps, dt_s, _ptr(psf), int(accumulate), _stream()))
         return psf
 
     def strehl(self, psf, n_exposures: float):

@@ -2,6 +2,7 @@
 // Validation, device tables, workspace planning and launch sequencing only; every number of
 // the forward model is produced by the kernels in k_*.cu.
 #include <cmath>
+#include <complex>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -55,6 +56,18 @@ static cudaError_t build_group(ao_geometry* g, Group& grp)
     return upload(&grp.d_off_stage, off_stage.data(), off_stage.size());
 }
 
+static void free_sodium(WfsH& w)
+{
+    cudaFree((void*)w.na.rho); cudaFree((void*)w.na.gturn); cudaFree((void*)w.na.launch);
+    w.na = SodiumP();
+}
+
+static void free_band(ao_geometry* g)
+{
+    cudaFree(g->band.d_tw); cudaFree(g->band.d_cin); cudaFree(g->band.d_Hf); cudaFree(g->band.d_cout);
+    g->band = PsfBand();
+}
+
 static void free_group(Group& grp)
 {
     cudaFree(grp.d_src); cudaFree(grp.d_off_api); cudaFree(grp.d_off_stage);
@@ -66,11 +79,13 @@ static void destroy(ao_geometry* g)
     if (!g) return;
     cudaFree(g->d_pupil_amp); cudaFree(g->d_layers); cudaFree(g->d_sources);
     cudaFree(g->d_psf_tw); cudaFree(g->d_psf_pre);
+    free_band(g);
     if (g->ev_fork) cudaEventDestroy(g->ev_fork);
     if (g->ev_join) cudaEventDestroy(g->ev_join);
     if (g->side) cudaStreamDestroy(g->side);
     for (auto& w : g->wfs) {
         cudaFree(w.d_amp); cudaFree(w.d_valid); cudaFree(w.d_w2m); cudaFree(w.d_tw); cudaFree(w.d_twf); cudaFree(w.d_pre); cudaFree(w.fused_items);
+        free_sodium(w);
         free_group(w.grp);
     }
     free_group(g->all); free_group(g->sci);
@@ -169,7 +184,8 @@ static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0
             return AO_OK;
         }
     }
-    const bool need_ws = (phase_dev == nullptr) || w.big;
+    const bool big = w.big && !(w.na.n_z > 0 && w.M <= 64);     // an extended beacon at M = 64 runs k_sh_generic
+    const bool need_ws = (phase_dev == nullptr) || big;
     if (need_ws && (!g->ws || g->ws_chunk < 1))
         return fail(AO_ERR_WORKSPACE, "workspace required (phase_dev == NULL or fft > 64): call ao_set_workspace");
     const NoiseP nz = make_noise(noise);
@@ -186,7 +202,7 @@ static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0
         }
         float* img = images ? images + (size_t)c0 * n_sel * nsa * PP : nullptr;
         float* slp = slopes ? slopes + (size_t)c0 * n_sel * 2 * nsa : nullptr;
-        if (!w.big) {
+        if (!big) {
             AO_CUDA(launch_sh_small(g, w, ph, api, stride, step0 + c0, ks, nz, img, slp, st), "sh_small");
         } else {
             float* im = img ? img : v.bigimg;
@@ -199,9 +215,10 @@ static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0
 }
 
 static int run_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, double dt,
-                   float* psf, int accumulate, cudaStream_t st)
+                   float* psf, int accumulate, cudaStream_t st, bool poly = false)
 {
     if (g->sci.src.empty() || !g->psf_fft) return fail(AO_ERR_INVALID_ARG, "no science direction / psf_fft == 0");
+    if (poly && g->band.n == 0) return fail(AO_ERR_INVALID_ARG, "ao_psf_poly: no wavelength band set (ao_set_psf_band)");
     if (!g->ws || g->ws_chunk < 1) return fail(AO_ERR_WORKSPACE, "ao_psf needs a workspace: call ao_set_workspace");
     const WsView v = ws_view(g);
     if (n_steps == 0 && !accumulate) {
@@ -220,6 +237,11 @@ static int run_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_
         const int kc = psf_chunk_steps(g);
         for (int k = 0; k < ks; k += kc) {
             const int kn = ks - k < kc ? ks - k : kc;
+            if (poly) {
+                for (int j = 0; j < g->band.n; ++j)
+                    AO_CUDA(launch_psf_poly(g, ph + (size_t)k * stride, api, stride, kn, j, v.scratch, psf,
+                                            (accumulate || c0 + k > 0 || j > 0) ? 1 : 0, st), "psf_poly");
+            } else
             AO_CUDA(launch_psf(g, ph + (size_t)k * stride, api, stride, kn, v.scratch, psf,
                                (accumulate || c0 + k > 0) ? 1 : 0, st), "psf");
         }
@@ -360,11 +382,12 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
             if ((e = upload(&d, items.data(), items.size())) != cudaSuccess) return bail("fused items upload");
             w.fused_items = d;
         }
-        if (!w.big) {
+        if (w.M <= 64) {      // direct-DFT table of k_sh_generic (M = 64 uses it for extended beacons only)
             std::vector<float2> t(2 * w.M);
             for (int q = 0; q < 2 * w.M; ++q) t[q] = make_float2((float)cos(PI * q / w.M), (float)(-sin(PI * q / w.M)));
             if ((e = upload(&w.d_w2m, t.data(), t.size())) != cudaSuccess) return bail("twiddle upload");
-        } else {
+        }
+        if (w.big) {
             std::vector<float2> t(w.M / 2), pr(w.n);
             for (int k = 0; k < w.M / 2; ++k) t[k] = make_float2((float)cos(2 * PI * k / w.M), (float)(-sin(2 * PI * k / w.M)));
             for (int a = 0; a < w.n; ++a) {
@@ -547,7 +570,7 @@ static int forward_chunk(ao_geometry* g, int64_t step0, int n_steps, double dt_s
             rc = run_wfs(g, (int)wi, nullptr, step0, n_steps, dt_s, noise, nullptr, slopes[wi], on_side[wi] ? sw : st);
         }
         if (pass == 0 && want_psf && rc == AO_OK)
-            rc = run_psf(g, nullptr, step0, n_steps, dt_s, psf, accumulate, sw);
+            rc = run_psf(g, nullptr, step0, n_steps, dt_s, psf, accumulate, sw, g->band.n > 0);
     }
     // the side stream is joined on every path, also after a failed launch: work already queued there must stay
     // ordered before whatever the caller submits next on `st`
@@ -566,6 +589,125 @@ int ao_set_phase_map(ao_geometry* g, int source, const float* map_dev)
     AO_CUDA(cudaDeviceSynchronize(), "synchronize before the source table update");
     g->sources[source].map = map_dev;
     AO_CUDA(cudaMemcpy(g->d_sources + source, &g->sources[source], sizeof(SourceP), cudaMemcpyHostToDevice), "source table update");
+    return AO_OK;
+}
+
+// radix-2 FFT in FP64 on the host (tables of the chirp-z transform only)
+static void host_fft(std::vector<std::complex<double>>& x)
+{
+    const size_t n = x.size();
+    for (size_t i = 1, j = 0; i < n; ++i) {
+        size_t bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) std::swap(x[i], x[j]);
+    }
+    const double PI = 3.14159265358979323846;
+    for (size_t len = 2; len <= n; len <<= 1)
+        for (size_t base = 0; base < n; base += len)
+            for (size_t k = 0; k < len / 2; ++k) {
+                const std::complex<double> w = std::polar(1.0, -2.0 * PI * (double)k / (double)len);
+                const std::complex<double> u = x[base + k], t = w * x[base + k + len / 2];
+                x[base + k] = u + t; x[base + k + len / 2] = u - t;
+            }
+}
+
+int ao_set_psf_band(ao_geometry* g, const double* lambdas_m_host, const double* weights_host, int n_lambda)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (n_lambda < 0 || n_lambda > 256 || (n_lambda > 0 && (!lambdas_m_host || !weights_host)))
+        return fail(AO_ERR_INVALID_ARG, "ao_set_psf_band: need 0 <= n_lambda <= 256 and non-NULL arrays");
+    if (n_lambda > 0 && (g->sci.src.empty() || !g->psf_fft)) return fail(AO_ERR_INVALID_ARG, "ao_set_psf_band: no science direction / psf_fft == 0");
+    const int M = g->psf_fft, Np = g->Np;
+    int logL = 8;
+    while ((1 << logL) < M + Np - 1) ++logL;
+    if (n_lambda > 0 && logL > 12) return fail(AO_ERR_UNSUPPORTED, "ao_set_psf_band: psf_fft + pupil n - 1 must not exceed 4096");
+    double lambda_s = 0.0;
+    for (size_t i = 0; i < g->sci.src.size() && n_lambda > 0; ++i) {
+        const double l = g->lambda_ref / g->sources[g->sci.src[i]].scale;
+        if (i == 0) lambda_s = l;
+        else if (fabs(l - lambda_s) > 1e-12 * lambda_s) return fail(AO_ERR_UNSUPPORTED, "ao_set_psf_band: the science directions must share one wavelength");
+    }
+    for (int j = 0; j < n_lambda; ++j)
+        if (!(lambdas_m_host[j] > 0)) return fail(AO_ERR_INVALID_ARG, "ao_set_psf_band: wavelengths must be positive");
+    AO_CUDA(cudaDeviceSynchronize(), "synchronize before the band table update");
+    free_band(g);
+    if (n_lambda == 0) return AO_OK;
+    const int L = 1 << logL;
+    const double PI = 3.14159265358979323846;
+    auto cis_turns = [&](double t) { t -= floor(t); return std::polar(1.0, 2.0 * PI * t); };     // exp(2 pi i t), reduced in FP64
+    std::vector<float2> tw(L), cin((size_t)n_lambda * Np), Hf((size_t)n_lambda * L), cout((size_t)n_lambda * M);
+    for (int k = 0; k < L; ++k) tw[k] = make_float2((float)cos(2 * PI * k / L), (float)(-sin(2 * PI * k / L)));
+    PsfBand B;
+    B.n = n_lambda; B.L = L; B.logL = logL;
+    for (int j = 0; j < n_lambda; ++j) {
+        const double s = lambda_s / lambdas_m_host[j];
+        B.scale.push_back(s); B.weight.push_back(weights_host[j]);
+        for (int b = 0; b < Np; ++b) {          // exp(-i pi s b^2 / M) = exp(2 pi i (-s b^2 / (2M)))
+            const std::complex<double> c = cis_turns(-s * (double)b * b / (2.0 * M));
+            cin[(size_t)j * Np + b] = make_float2((float)c.real(), (float)c.imag());
+        }
+        for (int k = 0; k < M; ++k) {
+            const double kap = (double)k - 0.5 * M;
+            const std::complex<double> c = cis_turns(-s * kap * kap / (2.0 * M));
+            cout[(size_t)j * M + k] = make_float2((float)c.real(), (float)c.imag());
+        }
+        std::vector<std::complex<double>> h(L, 0.0);
+        for (int u = -(Np - 1); u <= M - 1; ++u) {
+            const double t = (double)u - 0.5 * M;
+            h[(size_t)((u % L + L) % L)] = cis_turns(s * t * t / (2.0 * M));
+        }
+        host_fft(h);
+        for (int i = 0; i < L; ++i) Hf[(size_t)j * L + i] = make_float2((float)(h[i].real() / L), (float)(h[i].imag() / L));
+    }
+    cudaError_t e = upload(&B.d_tw, tw.data(), tw.size());
+    if (e == cudaSuccess) e = upload(&B.d_cin, cin.data(), cin.size());
+    if (e == cudaSuccess) e = upload(&B.d_Hf, Hf.data(), Hf.size());
+    if (e == cudaSuccess) e = upload(&B.d_cout, cout.data(), cout.size());
+    g->band = B;
+    if (e != cudaSuccess) { free_band(g); return cuda_fail(e, "band table upload"); }
+    return AO_OK;
+}
+
+int ao_psf_poly(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, double dt_s, float* psf_dev,
+                int accumulate, void* cuda_stream)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (!psf_dev || n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_psf_poly: psf_dev NULL or n_steps < 0");
+    return run_psf(g, phase_dev, step0, n_steps, dt_s, psf_dev, accumulate, (cudaStream_t)cuda_stream, true);
+}
+
+int ao_set_sodium(ao_geometry* g, int wfs_index, int n_z, const double* z_m_host, const double* rho_host, int n_t,
+                  const double* launch_xy_m_host)
+{
+    int rc = check_entry(g); if (rc) return rc;
+    if (wfs_index < 0 || wfs_index >= (int)g->wfs.size()) return fail(AO_ERR_INVALID_ARG, "ao_set_sodium: wfs_index out of range");
+    WfsH& w = g->wfs[wfs_index];
+    if (n_z < 0 || n_z > 64 || (n_z > 0 && (n_t < 1 || !z_m_host || !rho_host || !launch_xy_m_host)))
+        return fail(AO_ERR_INVALID_ARG, "ao_set_sodium: need 0 <= n_z <= 64 and, for n_z > 0, n_t >= 1 and non-NULL arrays");
+    if (n_z > 0 && w.M > 64) return fail(AO_ERR_UNSUPPORTED, "ao_set_sodium: extended beacons are implemented for sensors with fft <= 64");
+    const size_t n_sel = w.grp.src.size();
+    std::vector<double> gt(n_sel * (size_t)n_z);
+    for (size_t si = 0; si < n_sel && n_z > 0; ++si) {
+        const SourceP& sp = g->sources[w.grp.src[si]];
+        const double lambda_s = g->lambda_ref / sp.scale;
+        if (std::isinf(sp.H)) return fail(AO_ERR_INVALID_ARG, "ao_set_sodium: a source of this sensor is at infinity");
+        for (int iz = 0; iz < n_z; ++iz) {
+            if (!(z_m_host[iz] > 0)) return fail(AO_ERR_INVALID_ARG, "ao_set_sodium: altitudes must be positive");
+            gt[si * n_z + iz] = (1.0 / sp.H - 1.0 / z_m_host[iz]) * sp.d / lambda_s;
+        }
+    }
+    AO_CUDA(cudaDeviceSynchronize(), "synchronize before the sodium table update");
+    free_sodium(w);
+    if (n_z == 0) return AO_OK;
+    std::vector<float> rho((size_t)n_t * n_z);
+    for (size_t i = 0; i < rho.size(); ++i) rho[i] = (float)rho_host[i];
+    float* d_rho = nullptr; double* d_g = nullptr; double* d_l = nullptr;
+    cudaError_t e = upload(&d_rho, rho.data(), rho.size());
+    if (e == cudaSuccess) e = upload(&d_g, gt.data(), gt.size());
+    if (e == cudaSuccess) e = upload(&d_l, launch_xy_m_host, 2 * n_sel);
+    if (e != cudaSuccess) { cudaFree(d_rho); cudaFree(d_g); cudaFree(d_l); return cuda_fail(e, "sodium table upload"); }
+    w.na.n_z = n_z; w.na.n_t = n_t; w.na.rho = d_rho; w.na.gturn = d_g; w.na.launch = d_l;
     return AO_OK;
 }
 

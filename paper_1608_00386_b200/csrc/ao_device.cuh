@@ -91,6 +91,39 @@ __device__ __forceinline__ void sincos_reduced(const float x, float* s, float* c
     *c = __cosf(a);
 }
 
+// Reading O9: phase ramp of scatterer iz for the subaperture (p, q) of source-of-WFS si, in 0.32 fixed-point turns per
+// sample: tau = gturn (c - L), c the subaperture centre on the O1 grid.  FP64 up to the fractional part.
+__device__ __forceinline__ ElongRamp elong_ramp(const SodiumP& na, const int si, const int iz, const int p, const int q,
+                                                const int n, const int N, const double d)
+{
+    const double g = na.gturn[si * na.n_z + iz];
+    const double xc = (((double)(q * n) + 0.5 * (double)(n - 1)) - 0.5 * (double)(N - 1)) * d;
+    const double yc = (((double)(p * n) + 0.5 * (double)(n - 1)) - 0.5 * (double)(N - 1)) * d;
+    const double tx = g * (xc - na.launch[2 * si]), ty = g * (yc - na.launch[2 * si + 1]);
+    ElongRamp r;
+    r.fx = (uint32_t)__double2ull_rn((tx - floor(tx)) * 4294967296.0);
+    r.fy = (uint32_t)__double2ull_rn((ty - floor(ty)) * 4294967296.0);
+    return r;
+}
+
+// cos and sin of 2 pi t for t in 0.32 fixed-point turns (wrap-around is exact; SFU on [-pi, pi]).
+__device__ __forceinline__ void sincos_turns(const uint32_t t, float* s, float* c)
+{
+    const float a = (float)(int32_t)t * (6.283185307179586f * 2.3283064365386963e-10f);
+    *s = __sinf(a);
+    *c = __cosf(a);
+}
+
+// A phase in radians as 0.32 fixed-point turns (same two-constant reduction as sincos_reduced).
+__device__ __forceinline__ uint32_t phase_to_turns(const float x)
+{
+    const float kInv2PiHi = 0.15915493667125702f, kInv2PiLo = 6.4206383266e-09f;
+    const float k = rintf(x * kInv2PiHi);
+    float r = fmaf(x, kInv2PiHi, -k);
+    r = fmaf(x, kInv2PiLo, r);                                  // [-1/2, 1/2] turns
+    return (uint32_t)__float2ll_rn(r * 4294967296.0f);
+}
+
 __device__ __forceinline__ float warp_sum(float v)
 {
 #pragma unroll

@@ -50,6 +50,17 @@ struct NoiseP {
     float photons, read_noise;
 };
 
+// Extended sodium layer of the LGS sensors of one WFS (ao_set_sodium; DESIGN.md section 3 reading O9).
+struct SodiumP {
+    int n_z = 0, n_t = 0;              // scatterers per profile, time samples of the profile (0: point beacon)
+    const float* rho = nullptr;        // [n_t][n_z] weights, device
+    const double* gturn = nullptr;     // [n_sel][n_z]: (1/H_s - 1/z) d_s / lambda_s, turns per sample per metre of baseline
+    const double* launch = nullptr;    // [n_sel][2] launch point, metres in the pupil plane
+};
+
+// Spot shift of one scatterer as a phase ramp in 0.32 fixed-point turns per sample (exact wrap-around arithmetic).
+struct ElongRamp { uint32_t fx, fy; };
+
 struct WfsH {
     int n_sub, n, M, beta, P;
     float min_illum;
@@ -63,9 +74,20 @@ struct WfsH {
     float2* d_tw = nullptr;         // exp(-2 pi i k / M), k < M/2         (big path, generic fallback)
     float2* d_twf = nullptr;        // exp(-2 pi i k / M), k < M           (big path, Stockham passes)
     float2* d_pre = nullptr;        // pre-twiddle exp(+i pi (M-1) a / M), a < n  (big path)
+    SodiumP na;                     // extended beacon (device pointers owned by the handle), n_z = 0: none
     void* fused_items = nullptr;    // device WorkItem[]: runs of <= fused_G adjacent valid subapertures
     int n_fused_items = 0, fused_G = 0, fused_R2 = 0;
     Group grp;
+};
+
+// Wavelength band of the polychromatic science PSF (ao_set_psf_band; reading O8): chirp-z tables per wavelength.
+struct PsfBand {
+    int n = 0, L = 0, logL = 0;             // wavelengths, FFT length of the circular convolution (>= M + Np - 1)
+    std::vector<double> scale, weight;      // s_j = lambda_s / lambda_j, w_j
+    float2* d_tw = nullptr;                 // exp(-2 pi i k / L), k < L
+    float2* d_cin = nullptr;                // [n][Np]  exp(-i pi s b^2 / M)
+    float2* d_Hf = nullptr;                 // [n][L]   FFT_L(h) / L, h[u] = exp(+i pi s (u - M/2)^2 / M)
+    float2* d_cout = nullptr;               // [n][M]   exp(-i pi s (k' - M/2)^2 / M)
 };
 
 }  // namespace ao
@@ -85,6 +107,7 @@ struct ao_geometry {
     float2* d_psf_tw = nullptr;       // exp(-2 pi i k / M), k < M
     float2* d_psf_pre = nullptr;      // (-1)^a as a complex table, a < Np
     ao::Group all, sci;
+    ao::PsfBand band;                 // n = 0: no band set
     long long phase_elems_per_step = 0;
     // workspace
     char* ws = nullptr;
@@ -130,6 +153,9 @@ cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, boo
 cudaError_t launch_psf(ao_geometry* g, const float* phase, bool api_layout, long long step_stride,
                        int ks, float2* scratch, float* psf, int accumulate, cudaStream_t st);
 int psf_chunk_steps(const ao_geometry* g);
+// polychromatic PSF: wavelength j of the band, ks <= psf_chunk_steps(g) steps added into psf (k_psf_poly.cu)
+cudaError_t launch_psf_poly(ao_geometry* g, const float* phase, bool api_layout, long long step_stride, int ks,
+                            int j, float2* scratch, float* psf, int accumulate, cudaStream_t st);
 bool sh_big_fast(const WfsH& w);                                    // the Stockham two-pass path applies (else generic)
 
 // fused trace + SH + CoG (k_fused.cu); cudaErrorNotSupported if the geometry is outside its fast path

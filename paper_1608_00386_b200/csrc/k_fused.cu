@@ -63,6 +63,7 @@ struct FusedArgs {
     NoiseP nz;
     float* images;                    // nullable [k][si][nsa][P][P]
     float* slopes;                    // nullable [k][si][2][nsa]
+    SodiumP na;                       // extended beacon (ELONG kernels only; reading O9)
 };
 
 
@@ -82,7 +83,7 @@ struct FusedCfg {
     static_assert(kTR % n == 0 && NT % n == 0 && n <= 32, "bad fused configuration");
 };
 
-template <int M, bool NOISE, bool ANYDU, bool MAPS>
+template <int M, bool NOISE, bool ANYDU, bool MAPS, bool ELONG>
 __global__ void __launch_bounds__(kFusedThreads, 4)
 k_fused(const FusedArgs A)
 {
@@ -125,10 +126,46 @@ k_fused(const FusedArgs A)
         const int sa = inb ? p * A.n_sub + q : 0;
         const bool active = inb && A.valid[sa] != 0;
         if (!__any_sync(0xffffffffu, active)) continue;
-        __syncwarp();                                      // the previous round has finished reading xs
+        float binacc[2][P];                                // the two detector-row groups of this thread, before the exchange
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+            for (int i = 0; i < P; ++i) binacc[hh][i] = 0.0f;
+        const float* ap = A.amp + (size_t)(p * n) * N + (size_t)q * n + b;
+        uint32_t pht[ELONG ? n : 1];                       // ELONG: phase of the thread's column in 0.32 fixed-point turns
+        if (ELONG) {
+#pragma unroll
+            for (int i = 0; i < n; ++i) {
+                u64 v = acc[i];
+#pragma unroll
+                for (int hh = 1; hh < K::HS; ++hh) v = (hs == hh) ? acc[hh * n + i] : v;
+                const float2 f = unpack2(v);
+                float ph = (c ? f.y : f.x) * scale;
+                if (MAPS && mp && active) ph += __ldg(mp + (size_t)(p * n + i) * N + (size_t)q * n + b);
+                pht[ELONG ? i : 0] = phase_to_turns(ph);
+            }
+        }
+        const int n_z = ELONG ? A.na.n_z : 1;
+        const float* rho = ELONG ? A.na.rho + (size_t)((A.T.step0 + k) % A.na.n_t) * A.na.n_z : nullptr;
+#pragma unroll 1
+        for (int iz = 0; iz < n_z; ++iz) {
+        __syncwarp();                                      // the previous round / scatterer has finished reading xs
+        float wz = 1.0f;
         {
             float2 e[n];
-            const float* ap = A.amp + (size_t)(p * n) * N + (size_t)q * n + b;
+            if (ELONG) {                                   // E = A exp(i (phi + ramp of scatterer iz)), reading O9
+                const ElongRamp rp = elong_ramp(A.na, si, iz, p, q, n, N, sp.d);
+                wz = __ldg(rho + iz);
+                uint32_t t = (uint32_t)b * rp.fx;
+#pragma unroll
+                for (int i = 0; i < n; ++i) {
+                    const float Am = active ? __ldg(ap + (size_t)i * N) : 0.0f;
+                    float s, co;
+                    sincos_turns(pht[ELONG ? i : 0] + t, &s, &co);
+                    e[i] = make_float2(Am * co, Am * s);
+                    t += rp.fy;
+                }
+            } else {
 #pragma unroll
             for (int i = 0; i < n; ++i) {
                 u64 v = acc[i];
@@ -142,6 +179,7 @@ k_fused(const FusedArgs A)
                 sincos_reduced(ph, &s, &co);
                 e[i] = make_float2(Am * co, Am * s);
             }
+            }
             dft_half_padded<M>(e, [&](auto ki, const float2 v) {
                 constexpr int kk = decltype(ki)::value;
                 xs[kk * K::XP + b] = v;                    // column FFT result: T[k][b]
@@ -149,8 +187,6 @@ k_fused(const FusedArgs A)
         }
         __syncwarp();
         // rows k = b and k = b + n of this subaperture
-        float pixv[2][P];
-        int cbase = 0;
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
             const int kr = b + hh * n;
@@ -164,6 +200,17 @@ k_fused(const FusedArgs A)
                 constexpr int m = decltype(mi)::value;
                 bins[m / BETA] = fmaf(v.x, v.x, fmaf(v.y, v.y, bins[m / BETA]));
             });
+#pragma unroll
+            for (int i = 0; i < P; ++i) binacc[hh][i] = ELONG ? fmaf(wz, bins[i], binacc[hh][i]) : bins[i];
+        }
+        }
+        float pixv[2][P];
+        int cbase = 0;
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            float bins[P];
+#pragma unroll
+            for (int i = 0; i < P; ++i) bins[i] = binacc[hh][i];
             // sum the BETA rows of a detector row: halving exchange among BETA adjacent threads
             int cnt = P; cbase = 0;
 #pragma unroll
@@ -244,10 +291,13 @@ static cudaError_t launch_fused_variant(ao_geometry* g, const WfsH& w, FusedArgs
     bool maps = false;                                     // the map-free kernel keeps its register budget
     for (int si : w.grp.src) maps = maps || g->sources[si].map != nullptr;
     void (*kern)(const FusedArgs);
-    if (maps) kern = pl.anydu ? (a.nz.on ? k_fused<M, true, true, true> : k_fused<M, false, true, true>)
-                              : (a.nz.on ? k_fused<M, true, false, true> : k_fused<M, false, false, true>);
-    else kern = pl.anydu ? (a.nz.on ? k_fused<M, true, true, false> : k_fused<M, false, true, false>)
-                         : (a.nz.on ? k_fused<M, true, false, false> : k_fused<M, false, false, false>);
+    if (a.na.n_z > 0)       // extended beacon: its own instantiations (they also read the phase maps if any are set)
+        kern = pl.anydu ? (a.nz.on ? k_fused<M, true, true, true, true> : k_fused<M, false, true, true, true>)
+                        : (a.nz.on ? k_fused<M, true, false, true, true> : k_fused<M, false, false, true, true>);
+    else if (maps) kern = pl.anydu ? (a.nz.on ? k_fused<M, true, true, true, false> : k_fused<M, false, true, true, false>)
+                                   : (a.nz.on ? k_fused<M, true, false, true, false> : k_fused<M, false, false, true, false>);
+    else kern = pl.anydu ? (a.nz.on ? k_fused<M, true, true, false, false> : k_fused<M, false, true, false, false>)
+                         : (a.nz.on ? k_fused<M, true, false, false, false> : k_fused<M, false, false, false, false>);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     const size_t nsa = (size_t)w.n_sub * w.n_sub;
@@ -285,7 +335,7 @@ cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_ste
     a.items = (const WorkItem*)w.fused_items; a.n_items = w.n_fused_items; a.n_steps = n_steps;
     a.amp = w.d_amp; a.valid = w.d_valid; a.n_sub = w.n_sub;
     a.norm = (float)(1.0 / ((double)w.M * w.M * (double)w.n * w.n));
-    a.nz = noise; a.images = images; a.slopes = slopes;
+    a.nz = noise; a.images = images; a.slopes = slopes; a.na = w.na;
     if (w.M == 32) return launch_fused_variant<32>(g, w, a, pl, n_steps, st);
     return launch_fused_variant<16>(g, w, a, pl, n_steps, st);
 }

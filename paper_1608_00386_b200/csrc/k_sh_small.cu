@@ -17,8 +17,8 @@ __global__ void __launch_bounds__(256)
 k_sh_generic(const float* __restrict__ phase, long long step_stride, const long long* __restrict__ off,
              const int* __restrict__ sel, int n_sel, const float* __restrict__ amp,
              const uint8_t* __restrict__ valid, const float2* __restrict__ w2m, int n_sub, int n, int M,
-             int beta, int P, float norm, NoiseP nz, long long step0, float* __restrict__ images,
-             float* __restrict__ slopes)
+             int beta, int P, float norm, NoiseP nz, long long step0, const SodiumP na, const double d_grid,
+             float* __restrict__ images, float* __restrict__ slopes)
 {
     extern __shared__ float4 smem_raw[];
     const int sa = blockIdx.x, si = blockIdx.y, k = blockIdx.z;
@@ -38,45 +38,68 @@ k_sh_generic(const float* __restrict__ phase, long long step_stride, const long 
     float2* R = E + n * n;                                      // [n][W]   (window columns only)
     float* I = reinterpret_cast<float*>(R + n * W);             // [W][W]
     float* pix = I + W * W;                                     // [P][P]
+    float2* E0 = reinterpret_cast<float2*>(pix + PP);           // [n][n]  (amplitude, phase in turns): extended beacons only
     const int p = sa / n_sub, q = sa - p * n_sub, N = n_sub * n;
     const float* ph = phase + (size_t)k * step_stride + off[si];
     for (int i = tid; i < 2 * M; i += nt) Wt[i] = w2m[i];
+    const int n_z = na.n_z;                                     // 0: point beacon (one pass, no ramp)
     for (int i = tid; i < n * n; i += nt) {
         const int a = i / n, b = i - a * n;
         const size_t gidx = (size_t)(p * n + a) * N + q * n + b;
         const float A = amp[gidx];
-        float s, c;
-        sincosf(ph[gidx], &s, &c);
-        E[i] = make_float2(A * c, A * s);
+        if (n_z > 0) {
+            E0[i] = make_float2(A, __uint_as_float(phase_to_turns(ph[gidx])));
+        } else {
+            float s, c;
+            sincos_reduced(ph[gidx], &s, &c);
+            E[i] = make_float2(A * c, A * s);
+        }
     }
-    __syncthreads();
+    const float* rho = n_z > 0 ? na.rho + (size_t)((step0 + k) % na.n_t) * n_z : nullptr;
     const int twoM = 2 * M;
-    for (int i = tid; i < n * W; i += nt) {                     // rows
-        const int a = i / W, mw = i - a * W, m = k0 + mw;
-        int qs = (2 * m - M + 1) % twoM; if (qs < 0) qs += twoM;
-        int qi = 0;
-        float sr = 0.0f, sim = 0.0f;
-        for (int b = 0; b < n; ++b) {
-            const float2 x = E[a * n + b], w = Wt[qi];
-            sr = fmaf(x.x, w.x, fmaf(-x.y, w.y, sr));
-            sim = fmaf(x.x, w.y, fmaf(x.y, w.x, sim));
-            qi += qs; if (qi >= twoM) qi -= twoM;
+    for (int iz = 0; iz < (n_z > 0 ? n_z : 1); ++iz) {
+        float wz = 1.0f;
+        if (n_z > 0) {                                          // E = A exp(i (phi + ramp of scatterer iz)) (reading O9)
+            __syncthreads();                                    // E0 written / previous scatterer's E consumed
+            const ElongRamp rp = elong_ramp(na, si, iz, p, q, n, N, d_grid);
+            wz = rho[iz];
+            for (int i = tid; i < n * n; i += nt) {
+                const int a = i / n, b = i - a * n;
+                const float2 e0 = E0[i];
+                float s, c;
+                sincos_turns(__float_as_uint(e0.y) + (uint32_t)a * rp.fy + (uint32_t)b * rp.fx, &s, &c);
+                E[i] = make_float2(e0.x * c, e0.x * s);
+            }
         }
-        R[i] = make_float2(sr, sim);
-    }
-    __syncthreads();
-    for (int i = tid; i < W * W; i += nt) {                     // columns + intensity
-        const int kw = i / W, mw = i - kw * W, kk = k0 + kw;
-        int qs = (2 * kk - M + 1) % twoM; if (qs < 0) qs += twoM;
-        int qi = 0;
-        float sr = 0.0f, sim = 0.0f;
-        for (int a = 0; a < n; ++a) {
-            const float2 x = R[a * W + mw], w = Wt[qi];
-            sr = fmaf(x.x, w.x, fmaf(-x.y, w.y, sr));
-            sim = fmaf(x.x, w.y, fmaf(x.y, w.x, sim));
-            qi += qs; if (qi >= twoM) qi -= twoM;
+        __syncthreads();
+        for (int i = tid; i < n * W; i += nt) {                 // rows
+            const int a = i / W, mw = i - a * W, m = k0 + mw;
+            int qs = (2 * m - M + 1) % twoM; if (qs < 0) qs += twoM;
+            int qi = 0;
+            float sr = 0.0f, sim = 0.0f;
+            for (int b = 0; b < n; ++b) {
+                const float2 x = E[a * n + b], w = Wt[qi];
+                sr = fmaf(x.x, w.x, fmaf(-x.y, w.y, sr));
+                sim = fmaf(x.x, w.y, fmaf(x.y, w.x, sim));
+                qi += qs; if (qi >= twoM) qi -= twoM;
+            }
+            R[i] = make_float2(sr, sim);
         }
-        I[i] = (sr * sr + sim * sim) * norm;
+        __syncthreads();
+        for (int i = tid; i < W * W; i += nt) {                 // columns + intensity
+            const int kw = i / W, mw = i - kw * W, kk = k0 + kw;
+            int qs = (2 * kk - M + 1) % twoM; if (qs < 0) qs += twoM;
+            int qi = 0;
+            float sr = 0.0f, sim = 0.0f;
+            for (int a = 0; a < n; ++a) {
+                const float2 x = R[a * W + mw], w = Wt[qi];
+                sr = fmaf(x.x, w.x, fmaf(-x.y, w.y, sr));
+                sim = fmaf(x.x, w.y, fmaf(x.y, w.x, sim));
+                qi += qs; if (qi >= twoM) qi -= twoM;
+            }
+            const float v = (sr * sr + sim * sim) * norm;
+            I[i] = n_z > 0 ? fmaf(wz, v, iz ? I[i] : 0.0f) : v;
+        }
     }
     __syncthreads();
     for (int i = tid; i < PP; i += nt) {                        // binning (+ noise)
@@ -109,7 +132,7 @@ k_sh_generic(const float* __restrict__ phase, long long step_stride, const long 
 size_t sh_generic_smem(int n, int M, int beta, int P)
 {
     const size_t W = (size_t)beta * P;
-    return sizeof(float2) * (2 * M + (size_t)n * n + n * W) + sizeof(float) * (W * W + (size_t)P * P) + 16;
+    return sizeof(float2) * (2 * M + 2 * (size_t)n * n + n * W) + sizeof(float) * (W * W + (size_t)P * P) + 16;
 }
 
 cudaError_t launch_sh_small(ao_geometry* g, const WfsH& w, const float* phase, bool api_layout,
@@ -130,7 +153,7 @@ cudaError_t launch_sh_small(ao_geometry* g, const WfsH& w, const float* phase, b
         k_sh_generic<<<grid, 256, smem, st>>>(
             phase + (size_t)k0 * step_stride, step_stride, api_layout ? w.grp.d_off_api : w.grp.d_off_stage,
             w.grp.d_src, n_sel, w.d_amp, w.d_valid, w.d_w2m, w.n_sub, w.n, w.M, w.beta, w.P, norm, noise,
-            (long long)step0 + k0, images ? images + set0 * nsa * w.P * w.P : nullptr,
+            (long long)step0 + k0, w.na, g->sources[w.grp.src[0]].d, images ? images + set0 * nsa * w.P * w.P : nullptr,
             slopes ? slopes + set0 * 2 * nsa : nullptr);
         g->launches++;
         e = cudaGetLastError();

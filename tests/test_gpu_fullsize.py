@@ -137,6 +137,23 @@ def test_c2_full_size_noise_through_the_fused_kernel_and_ao_forward(c2_full):
            forward_slopes_off=n_off)
 
 
+def test_c2_full_size_lgs_elongation(c2_full):
+    """NEXT-3 at c2's full size: an extended sodium layer (5 scatterers, side launch, time-varying profile) through the
+    fused kernel, LGS 0 and LGS 3 in full against the oracle."""
+    import torch
+    cfg = c2_full
+    cfg.sodium = inputs.sodium_profile(cfg, n_z=5, n_t=8, launch="side")
+    try:
+        ref = oracle.forward(cfg, 13, 1, want_phase=False, sources=[0, 3])
+        geo = _geo(cfg, 1)
+        img, slp = geo.sh_images(0, None, 13, 1, cfg.dt_s)
+        torch.cuda.synchronize()
+        a = check_wfs(cfg, geo, ref, 0, img, slp, 1, "c2 full, elongated spots", sources=[0, 3])
+        report("c2_full_elongation", images_rel_l2=a[0], slopes_max_abs=a[1], per_subap_rel_l2=a[2])
+    finally:
+        cfg.sodium = None
+
+
 # ------------------------------------------------------------------------------------------------ c3
 def test_c3_full_size_ngs_sensors_and_two_science_psfs():
     """c3 as stated, one step: the three NGS sensors (2x2 subapertures of 480 samples, FFT 1024, 128x128 pixels) in

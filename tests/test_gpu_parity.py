@@ -485,3 +485,58 @@ def test_marechal_strehl_on_traced_phase():
     assert got.shape == want.shape
     assert np.abs(got - want).max() <= 1e-5
     assert (want > 0.01).all() and (want < 0.99).all(), want       # neither saturated nor trivial
+
+
+@pytest.mark.parametrize("M", [16, 32, 64])
+def test_lgs_spot_elongation_all_paths(M):
+    """NEXT-3 (reading O9): extended sodium layer with a time-varying profile and side launch.  The fused
+    kernel (M = 16, 32: k_fused<..., ELONG>), the phase-buffer path and M = 64 (k_sh_generic) against the oracle, over
+    steps that wrap the profile table; then the point beacon again after clearing the profile."""
+    import torch
+    cfg = inputs.make_config(4, n_sub=10, screen_n=1024, n_steps=3, lgs_fft=M, n_layers=6)
+    cfg.sources = cfg.sources[:6]; cfg.wfs = cfg.wfs[:1]; cfg.psf_fft = 0
+    cfg.sodium = inputs.sodium_profile(cfg, n_z=5, n_t=4, launch="side", fwhm_m=2e3)
+    ref = oracle.forward(cfg, 6, 3)
+    geo = _geo(cfg, 3)
+    img, slp = geo.sh_images(0, None, 6, 3, cfg.dt_s)
+    phase = geo.trace_layers(6, 3, cfg.dt_s)
+    img_p, slp_p = geo.sh_images(0, phase, 6, 3, cfg.dt_s)
+    torch.cuda.synchronize()
+    a = check_wfs(cfg, geo, ref, 0, img, slp, 3, f"elongation M={M}, phase_dev = NULL")
+    b = check_wfs(cfg, geo, ref, 0, img_p, slp_p, 3, f"elongation M={M}, phase buffer")
+    from tests.parity_util import report
+    report(f"elongation_M{M}", images_rel_l2=max(a[0], b[0]), slopes_max_abs=max(a[1], b[1]), per_subap_rel_l2=max(a[2], b[2]))
+    # the spots are longer than a point beacon's: the brightest pixel drops
+    cfg.sodium = None
+    point = oracle.forward(cfg, 6, 1, want_phase=False)
+    assert ref["images"][0][0].max() < point["images"][0][0].max()
+    geo.set_sodium(None)
+    img0, slp0 = geo.sh_images(0, None, 6, 1, cfg.dt_s)
+    torch.cuda.synchronize()
+    check_wfs(cfg, geo, point, 0, img0, slp0, 1, "point beacon after clearing the profile")
+
+
+def test_lgs_spot_elongation_with_noise_and_errors():
+    """Detector noise on elongated spots through the fused kernel (k_fused<32, NOISE, ..., ELONG>); ao_set_sodium rejects
+    sensors of natural stars and big-FFT sensors."""
+    import torch
+    from paper_1608_00386_b200 import binding
+    cfg = inputs.make_config(2, n_sub=9, screen_n=512, n_steps=1)
+    cfg.sodium = inputs.sodium_profile(cfg, n_z=3, n_t=1, fwhm_m=1.5e3)
+    ref = oracle.forward(cfg, 4, 1, want_phase=False, noise_on=True)
+    geo = _geo(cfg, 1)
+    noisy, slopes = geo.sh_images(0, None, 4, 1, cfg.dt_s, noise=cfg.noise)
+    torch.cuda.synchronize()
+    tot = bad = 0
+    for si, s in enumerate(cfg.sources_of_wfs(0)):
+        same = np.abs(noisy[0, si].cpu().numpy().astype(np.float64) - ref["noisy"][s][0]) < 0.5
+        tot += same.size; bad += int((~same).sum())
+        ok = same.reshape(same.shape[0], -1).all(axis=1)
+        d = np.abs(slopes[0, si].cpu().numpy().astype(np.float64) - ref["slopes"][s][0])
+        assert d[:, ok].max() <= SLOPE_TOL
+    assert bad <= max(1, int(1e-5 * tot))
+    c3 = inputs.make_config(3, n_sub=8, screen_n=512, n_steps=1)
+    g3 = _geo(c3, 1)
+    na = inputs.sodium_profile(c3, wfs_index=1, n_z=3, n_t=1)
+    with pytest.raises(binding.AoError):
+        g3.set_sodium(na)                                    # NGS sensor: sources at infinity / fft > 64
