@@ -268,6 +268,22 @@ def test_c4_full_size_ngs_sensor_and_science_psf(c4_screens):
     report("c4_full_ngs_psf", ngs_images_rel_l2=a[0], ngs_slopes_max_abs=a[1], ngs_per_subap_rel_l2=a[2], psf_rel_l2=e)
 
 
+def test_c4_full_size_polychromatic_psf(c4_screens):
+    """NEXT-4 at full size: the on-axis science PSF of c4 (960^2 pupil, 2048^2 pixels, chirp-z FFTs of 4096) over a
+    two-wavelength band, one step from the 8192^2 screens, against the oracle."""
+    import torch
+    cfg = _c4(c4_screens, 32)
+    cfg.psf_band = ([2.0e-6, 2.4e-6], [0.5, 0.5])
+    sci = cfg.science_sources()
+    refp = oracle.forward(cfg, 123, 1, want_phase=False, want_wfs=False, sources=sci)
+    geo = _geo(cfg, 1)
+    psf = geo.psf_poly(None, 123, 1, cfg.dt_s)
+    torch.cuda.synchronize()
+    e = rel_l2(psf[0].cpu().numpy(), refp["psf"][sci[0]])
+    assert e <= IMAGE_TOL, e
+    report("c4_full_psf_poly", psf_rel_l2=e)
+
+
 # ------------------------------------------------------------------------------------------------ fallbacks
 def test_big_fft_generic_fallback_and_noise_on_a_big_sensor():
     """(i) A big-FFT sensor whose bin factor is not a power of two (beta = 6, FFT 128, 20x20 pixels of the central

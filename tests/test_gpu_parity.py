@@ -540,3 +540,45 @@ def test_lgs_spot_elongation_with_noise_and_errors():
     na = inputs.sodium_profile(c3, wfs_index=1, n_z=3, n_t=1)
     with pytest.raises(binding.AoError):
         g3.set_sodium(na)                                    # NGS sensor: sources at infinity / fft > 64
+
+
+@pytest.mark.parametrize("n_sub,n_steps", [(8, 3), (20, 2)])
+def test_polychromatic_psf_against_the_oracle(n_sub, n_steps):
+    """NEXT-4 (reading O8): ao_psf_poly over a three-wavelength band (chirp-z scaled DFTs on the pixel grid
+    of the directions' own wavelength) against the oracle's F E F^T definition; from a phase buffer and with the library's
+    own ray-trace, accumulating, through ao_forward, and one wavelength = ao_psf."""
+    import torch
+    cfg = inputs.make_config(3, n_sub=n_sub, screen_n=512, n_steps=n_steps)
+    cfg.sources = cfg.sources[:9] + cfg.sources[9:12]                 # three science directions are enough
+    cfg.psf_band = ([1.9e-6, 2.2e-6, 2.45e-6], [0.25, 0.45, 0.30])
+    sci = cfg.science_sources()
+    ref = oracle.forward(cfg, 2, n_steps, want_phase=False, want_wfs=False, sources=sci)
+    geo = _geo(cfg, n_steps)
+    p = geo.psf_poly(None, 2, n_steps, cfg.dt_s)
+    phase = geo.trace_layers(2, n_steps, cfg.dt_s)
+    p2 = geo.psf_poly(phase, 2, n_steps, cfg.dt_s, psf=p.clone(), accumulate=True)
+    torch.cuda.synchronize()
+    worst = 0.0
+    for di, s in enumerate(sci):
+        worst = max(worst, rel_l2(p[di].cpu().numpy(), ref["psf"][s]), rel_l2(p2[di].cpu().numpy(), 2.0 * ref["psf"][s]))
+    assert worst <= IMAGE_TOL, worst
+    from tests.parity_util import report
+    report(f"psf_poly_nsub{n_sub}", psf_rel_l2=worst)
+    # ao_forward uses the band while it is set
+    sl = [torch.empty((n_steps, len(cfg.sources_of_wfs(w)), 2, W.n_sub ** 2), dtype=torch.float32, device="cuda")
+          for w, W in enumerate(cfg.wfs)]
+    pf = torch.zeros_like(p)
+    geo.forward(2, n_steps, cfg.dt_s, sl, psf=pf)
+    torch.cuda.synchronize()
+    assert torch.allclose(pf, p, rtol=1e-6, atol=0.0)
+    # a band of the directions' own wavelength alone is the monochromatic PSF (two different transforms: chirp-z, FFT)
+    geo.set_psf_band([2.2e-6], [1.0])
+    mono = geo.psf(None, 2, n_steps, cfg.dt_s)
+    one = geo.psf_poly(None, 2, n_steps, cfg.dt_s)
+    torch.cuda.synchronize()
+    for di in range(len(sci)):
+        assert rel_l2(one[di].cpu().numpy(), mono[di].cpu().numpy().astype(np.float64)) <= IMAGE_TOL
+    geo.set_psf_band(None)
+    from paper_1608_00386_b200 import binding
+    with pytest.raises(binding.AoError):
+        geo.psf_poly(None, 2, 1, cfg.dt_s)
