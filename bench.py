@@ -357,6 +357,54 @@ def run_gpu(args):
             sweep[str(M)] = {k: r2[k] for k in ("us_per_step", "frac", "achieved", "flop_per_subaperture_frame", "steps")}
             g2.close()
 
+    # ---- the widened rows, timed in the same run: NEXT-3 (extended sodium layer) and NEXT-4 (polychromatic PSF) ----
+    widened = {}
+    if not args.skip_sweep:
+        ks = min(K, 50)
+        geo.set_sodium(inputs.sodium_profile(cfg, n_z=5, n_t=8, launch="side"))
+        r3 = lgs_leg(geo, lgs, ks)
+        geo.set_sodium(None)
+        widened["next3_lgs_elongation"] = {"scatterers": 5, "us_per_step": r3["us_per_step"], "steps": ks,
+                                           "note": "LGS leg (ao_sh_images, phase_dev = NULL) with ao_set_sodium: 5 scatterers, side launch"}
+        band = ([2.0e-6, 2.2e-6, 2.4e-6], [0.3, 0.4, 0.3])
+        geo.set_psf_band(*band)
+        kp = min(K, 8)
+        p4 = torch.zeros_like(psf)
+        geo.psf_poly(None, first, kp, cfg.dt_s, psf=p4)
+        ts, _ = timed(lambda: geo.psf_poly(None, first, kp, cfg.dt_s, psf=p4, accumulate=True), R)
+        t_mono, _ = timed(lambda: geo.psf(None, first, kp, cfg.dt_s, psf=p4, accumulate=True), R)
+        geo.set_psf_band(None)
+        widened["next4_psf_poly"] = {"wavelengths": len(band[0]), "us_per_step": 1e6 * statistics.median(ts) / kp,
+                                     "us_per_step_monochromatic": 1e6 * statistics.median(t_mono) / kp, "steps": kp,
+                                     "note": f"ao_psf_poly (ray-trace + chirp-z, FFT 4096) against ao_psf, {cfg.psf_fft}^2 pixels, on-axis direction"}
+        del p4
+
+    # ---- the other workloads of BASELINE.json (c0 .. c3) at their stated sizes: full-step time of each ----
+    others = {}
+    if not args.skip_sweep:
+        for ci in (0, 1, 2, 3):
+            cc = inputs.make_config(ci, device=dev, keep_on_device=True)
+            nst = cc.n_steps
+            gc = binding.Geometry(cc, device=dev, workspace_steps=min(nst, batch))
+            slc = [torch.empty((nst, len(cc.sources_of_wfs(w)), 2, W.n_sub ** 2), dtype=torch.float32, device=dev)
+                   for w, W in enumerate(cc.wfs)]
+            pc = (torch.zeros((len(cc.science_sources()), cc.psf_fft, cc.psf_fft), dtype=torch.float32, device=dev)
+                  if cc.psf_fft else None)
+
+            def job():
+                for b0 in range(0, nst, batch):
+                    ksb = min(batch, nst - b0)
+                    gc.forward(b0, ksb, cc.dt_s, [t[b0:b0 + ksb] for t in slc], psf=pc, accumulate=True, noise=cc.noise)
+            job()
+            ts, nl = timed(job, max(3, R // 4), gc)
+            t = statistics.median(ts)
+            vf = sum(int(gc.wfs_valid(w).sum()) * len(cc.sources_of_wfs(w)) for w in range(len(cc.wfs)))
+            others[cc.name] = {"steps": nst, "ms_per_step": 1e3 * t / nst, "valid_subaperture_frames_per_step": vf,
+                               "subaperture_frames_per_sec": vf * nst / t, "launches": nl,
+                               "noise": cc.noise is not None, "science_psfs": len(cc.science_sources())}
+            gc.close()
+            del gc, slc, pc, cc
+
     # ---- optional: the residual-phase entry (NEXT-2), HBM-bound: every mode array is read once ----
     dm = None
     if args.dm_modes > 0:
@@ -441,7 +489,7 @@ def run_gpu(args):
                 "timing": {"repetitions": R, "statistic": "median over repetitions of the K-step region, CUDA events, max over ranks",
                            "ms_per_step_min": 1e3 * min(t_reps) / K, "ms_per_step_max": 1e3 * max(t_reps) / K},
                 "clocks": clocks, "gpu_launches": launches, "roofline": roofline, "e2e": e2e,
-                "cpu_baseline": cpu, "parity_spot_check": spot, "extra": {"sweep_lgs_leg": sweep},
+                "cpu_baseline": cpu, "parity_spot_check": spot, "extra": {"sweep_lgs_leg": sweep, "widened": widened, "other_configs_full_step": others},
                 "setup_seconds": t_setup,
                 "setup_note": f"{t_screens:.1f} s of it is the harness generating the 35 screens of 8192^2 (torch.fft), not the library"}
         if dm is not None:

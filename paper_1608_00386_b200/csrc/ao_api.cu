@@ -184,7 +184,9 @@ static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0
             return AO_OK;
         }
     }
-    const bool big = w.big && !(w.na.n_z > 0 && w.M <= 64);     // an extended beacon at M = 64 runs k_sh_generic
+    // M = 64 is grouped with the big sensors for its tables; it runs k_sh_reg (n = 32, 8 x 8 bins of the whole field),
+    // k_sh_generic for an extended beacon, else the one-CTA-per-subaperture Stockham kernel k_sh_mid64
+    const bool big = w.big && !(w.M <= 64 && (w.na.n_z > 0 || sh_reg_supported(w)));
     const bool need_ws = (phase_dev == nullptr) || big;
     if (need_ws && (!g->ws || g->ws_chunk < 1))
         return fail(AO_ERR_WORKSPACE, "workspace required (phase_dev == NULL or fft > 64): call ao_set_workspace");
@@ -203,7 +205,8 @@ static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0
         float* img = images ? images + (size_t)c0 * n_sel * nsa * PP : nullptr;
         float* slp = slopes ? slopes + (size_t)c0 * n_sel * 2 * nsa : nullptr;
         if (!big) {
-            AO_CUDA(launch_sh_small(g, w, ph, api, stride, step0 + c0, ks, nz, img, slp, st), "sh_small");
+            if (sh_reg_supported(w)) AO_CUDA(launch_sh_reg(g, w, ph, api, stride, step0 + c0, ks, nz, img, slp, st), "sh_reg");
+            else AO_CUDA(launch_sh_small(g, w, ph, api, stride, step0 + c0, ks, nz, img, slp, st), "sh_small");
         } else {
             float* im = img ? img : v.bigimg;
             AO_CUDA(launch_sh_big(g, w, ph, api, stride, ks, v.scratch, make_plan(g).scratch, im, st), "sh_big");

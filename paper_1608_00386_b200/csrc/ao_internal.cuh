@@ -131,6 +131,11 @@ cudaError_t launch_sh_small(ao_geometry* g, const WfsH& w, const float* phase, b
                             long long step_stride, int64_t step0, int n_steps, const NoiseP& noise,
                             float* images, float* slopes, cudaStream_t st);
 
+// in-register FFT path for M in {16, 24, 32}, n = M/2, full window (k_sh_reg.cu); other shapes: launch_sh_small
+bool sh_reg_supported(const WfsH& w);
+cudaError_t launch_sh_reg(ao_geometry* g, const WfsH& w, const float* phase, bool api_layout, long long step_stride,
+                          int64_t step0, int n_steps, const NoiseP& noise, float* images, float* slopes, cudaStream_t st);
+
 cudaError_t launch_centroids(ao_geometry* g, const WfsH& w, const float* images, int n_sets,
                              float* slopes, cudaStream_t st);
 

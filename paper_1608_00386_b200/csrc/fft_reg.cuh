@@ -110,4 +110,65 @@ __device__ __forceinline__ void fft_full_pk(float2 (&x)[N])
     }
 }
 
+// 12-point forward DFT in registers (3 x 4 Cooley-Tukey, compile-time twiddles), natural order in and out:
+// a = 4 a1 + a2, k = k1 + 3 k2:  X[k1 + 3 k2] = sum_a2 W4^(a2 k2) [ W12^(a2 k1) sum_a1 x[4 a1 + a2] W3^(a1 k1) ].
+__device__ __forceinline__ void fft12(float2 (&x)[12])
+{
+    float2 t[3][4];
+    static_for<0, 4>([&](auto a2i) {
+        constexpr int a2 = decltype(a2i)::value;
+        const float2 p = x[a2], q = x[4 + a2], r = x[8 + a2];
+        const float2 s = make_float2(q.x + r.x, q.y + r.y), d = make_float2(q.x - r.x, q.y - r.y);
+        const float2 m = make_float2(fmaf(-0.5f, s.x, p.x), fmaf(-0.5f, s.y, p.y));
+        const float h = 0.86602540378443864676f;                        // sqrt(3)/2; -i d = (d.y, -d.x)
+        const float2 t0 = make_float2(p.x + s.x, p.y + s.y);
+        const float2 t1 = make_float2(fmaf(h, d.y, m.x), fmaf(-h, d.x, m.y));
+        const float2 t2 = make_float2(fmaf(-h, d.y, m.x), fmaf(h, d.x, m.y));
+        t[0][a2] = t0;
+        t[1][a2] = cmul_cis<-a2, 6>(t1);                                 // W12^(a2 k1) = cis(-pi a2 k1 / 6)
+        t[2][a2] = cmul_cis<-2 * a2, 6>(t2);
+    });
+    static_for<0, 3>([&](auto k1i) {
+        constexpr int k1 = decltype(k1i)::value;
+        const float2 a = t[k1][0], b = t[k1][1], c = t[k1][2], d = t[k1][3];
+        const float2 ac = make_float2(a.x + c.x, a.y + c.y), amc = make_float2(a.x - c.x, a.y - c.y);
+        const float2 bd = make_float2(b.x + d.x, b.y + d.y), bmd = make_float2(b.x - d.x, b.y - d.y);
+        x[k1] = make_float2(ac.x + bd.x, ac.y + bd.y);
+        x[k1 + 6] = make_float2(ac.x - bd.x, ac.y - bd.y);
+        x[k1 + 3] = make_float2(amc.x + bmd.y, amc.y - bmd.x);           // - i (b - d)
+        x[k1 + 9] = make_float2(amc.x - bmd.y, amc.y + bmd.x);           // + i (b - d)
+    });
+}
+
+// Half-pixel-centred DFT of size M = 2n of n inputs (zero padded):
+//   X[k] = sum_a e[a] exp(-2 pi i (k - (M-1)/2) a / M),  k < M.
+// First DIF stage on the half-zero input: X[2k'] = FFT_n(e[a] cis(pi (M-1) a/M))[k'],
+//                                         X[2k'+1] = FFT_n(e[a] cis(pi (M-3) a/M))[k'].
+// `sink(k, value)` is called once for every k (k as std::integral_constant).
+template <int M, typename Sink>
+__device__ __forceinline__ void dft_half_padded(const float2 (&e)[M / 2], Sink&& sink)
+{
+    constexpr int n = M / 2;
+    if constexpr (n == 12) {                                           // M = 24 (workload c1): 12-point FFTs, 3 x 4
+        float2 y[n];
+        static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; y[a] = cmul_cis<(M - 1) * a, M>(e[a]); });
+        fft12(y);
+        static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k>{}, y[k]); });
+        static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; y[a] = cmul_cis<(M - 3) * a, M>(e[a]); });
+        fft12(y);
+        static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k + 1>{}, y[k]); });
+        return;
+    }
+    else {
+    u64 y[n];
+    static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; const float2 t = cmul_cis<(M - 1) * a, M>(e[a]); y[a] = pack2(t.x, t.y); });
+    fft_stage_pk<n, n / 2>(y);
+    static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k>{}, unpack2(y[bitrev_c(k, n)])); });
+    static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; const float2 t = cmul_cis<(M - 3) * a, M>(e[a]); y[a] = pack2(t.x, t.y); });
+    fft_stage_pk<n, n / 2>(y);
+    static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k + 1>{}, unpack2(y[bitrev_c(k, n)])); });
+    }
+}
+
+
 }  // namespace ao

@@ -31,24 +31,6 @@
 
 namespace ao {
 
-// Half-pixel-centred DFT of size M = 2n of n inputs (zero padded):
-//   X[k] = sum_a e[a] exp(-2 pi i (k - (M-1)/2) a / M),  k < M.
-// First DIF stage on the half-zero input: X[2k'] = FFT_n(e[a] cis(pi (M-1) a/M))[k'],
-//                                         X[2k'+1] = FFT_n(e[a] cis(pi (M-3) a/M))[k'].
-// `sink(k, value)` is called once for every k (k as std::integral_constant).
-template <int M, typename Sink>
-__device__ __forceinline__ void dft_half_padded(const float2 (&e)[M / 2], Sink&& sink)
-{
-    constexpr int n = M / 2;
-    u64 y[n];
-    static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; const float2 t = cmul_cis<(M - 1) * a, M>(e[a]); y[a] = pack2(t.x, t.y); });
-    fft_stage_pk<n, n / 2>(y);
-    static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k>{}, unpack2(y[bitrev_c(k, n)])); });
-    static_for<0, n>([&](auto ai) { constexpr int a = decltype(ai)::value; const float2 t = cmul_cis<(M - 3) * a, M>(e[a]); y[a] = pack2(t.x, t.y); });
-    fft_stage_pk<n, n / 2>(y);
-    static_for<0, n>([&](auto ki) { constexpr int k = decltype(ki)::value; sink(std::integral_constant<int, 2 * k + 1>{}, unpack2(y[bitrev_c(k, n)])); });
-}
-
 struct WorkItem { int p, q0, cnt, pad; };
 
 struct FusedArgs {
