@@ -71,9 +71,11 @@ cudaError_t launch_trace_tiled(ao_geometry* g, const Group& grp, bool api_layout
 {
     const int n_sel = (int)grp.src.size();
     if (n_sel == 0 || n_steps <= 0) return cudaSuccess;
-    const Tile2Plan p2 = plan_tiles2(g, grp.src, dt, 0);
+    // the phase writer has no exchange buffer to alias: three CTAs per SM (75 KB each) buy a third stage for the wide
+    // boxes of same-pitch grids (NGS sensors, science directions: du = 1, 22 KB per stage)
+    const Tile2Plan p2 = plan_tiles2(g, grp.src, dt, 0, 75 * 1024);
     if (p2.ok) {
-        auto kern2 = !p2.anydu ? k_trace_tiled2<0> : (p2.quad ? k_trace_tiled2<2> : k_trace_tiled2<1>);
+        auto kern2 = p2.unit ? k_trace_tiled2<3> : !p2.anydu ? k_trace_tiled2<0> : (p2.quad ? k_trace_tiled2<2> : k_trace_tiled2<1>);
         cudaError_t e2 = cudaFuncSetAttribute(kern2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p2.smem);
         if (e2 != cudaSuccess) return e2;
         TiledTrace2Args a;

@@ -90,6 +90,13 @@ __device__ __forceinline__ float lds_f32_next(uint32_t addr)
     asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v) : "r"(addr));
     return v;
 }
+template <int IMM>
+__device__ __forceinline__ float lds_f32_imm(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(addr), "n"(IMM));
+    return v;
+}
 __device__ __forceinline__ float4 lds_f32x4(uint32_t addr)
 {
     float4 v;

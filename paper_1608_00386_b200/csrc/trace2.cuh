@@ -21,7 +21,18 @@
 #include "ao_device.cuh"
 #include "pk_tma.cuh"
 
+#include <type_traits>
+
 namespace ao {
+
+template <int I, int N, typename F>
+__device__ __forceinline__ void static_for_t2(F&& f)
+{
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        static_for_t2<I + 1, N>(static_cast<F&&>(f));
+    }
+}
 
 constexpr int kTR = 16;                 // output rows of a tile
 constexpr int kKS = 2;                  // time steps per CTA
@@ -147,6 +158,33 @@ __device__ __forceinline__ void t2_march_quad(u64 (&acc)[kKS * kTR], const uint3
     }
 }
 
+// du == 1 exactly (grids with the screen pitch seen from infinity: the NGS sensors and the science directions): every
+// output row advances by one screen row and every column by one cell, so the bilinear weights are the same for the
+// whole tile and the box rows are consecutive: no table, and with the compile-time row pitch kUnitPitch every tap load
+// has an immediate offset.  acc_i += w0 X[r_0 + i] + w1 X[r_0 + i + 1].
+constexpr int kUnitPitch = 272;         // floats: 256 columns + wind shift of the paired step + alignment slack
+template <int ROW>
+__device__ __forceinline__ u64 t2_xrow_unit(const uint32_t a0, const uint32_t a1, const u64 fx, const u64 ref)
+{
+    constexpr int O = ROW * kUnitPitch * 4;
+    const u64 p0 = pack2(lds_f32_imm<O>(a0), lds_f32_imm<O>(a1));
+    const u64 p1 = pack2(lds_f32_imm<O + 4>(a0), lds_f32_imm<O + 4>(a1));
+    return fma2(fx, sub2(p1, p0), sub2(p0, ref));
+}
+template <int OFF>
+__device__ __forceinline__ void t2_march_unit(u64 (&acc)[kKS * kTR], const uint32_t tp0, const uint32_t tp1, const u64 fx,
+                                              const u64 ref, const float w0, const float w1)
+{
+    const u64 W0 = pack2(w0, w0), W1 = pack2(w1, w1);
+    u64 prev = t2_xrow_unit<0>(tp0, tp1, fx, ref);
+    static_for_t2<0, kTR>([&](auto ii) {
+        constexpr int i = decltype(ii)::value;
+        const u64 cur = t2_xrow_unit<i + 1>(tp0, tp1, fx, ref);
+        acc[OFF + i] = fma2(W1, cur, fma2(W0, prev, acc[OFF + i]));
+        prev = cur;
+    });
+}
+
 // Ray-trace one tile for two steps: rows ifirst .. ifirst+15, columns jfirst + {tid, tid + NT} of source `sp` at
 // time steps step_first and step_first + 1.  acc[s * 16 + i] receives the packed (column tid, column tid + NT)
 // layer sums of step s, row i, minus warp-uniform piston references (the same for both steps); with REFSUM
@@ -231,7 +269,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         const float* scr = T.scr;
         uint64_t* bar = &S.full_bar[stage];
         float* dst = tiles + (size_t)stage * tile_floats;
-        {   // row table of this stage: lane = step * 16 + row (FP64)
+        if (MODE != 3) {   // row table of this stage: lane = step * 16 + row (FP64); the unit march needs none
             static_assert(kKS * kTR == 32, "one lane per (step, row)");
             const int s = lane / kTR, i = lane - s * kTR;
             const double v = fma((double)i, T.du, T.vrel[s]);
@@ -309,7 +347,12 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         const u64 colA = (u64)(unsigned)tid * du64, colB = colA + (u64)NT * du64;
         const u64 colW = (u64)(unsigned)(tid & ~31) * du64;
         if (!AO_DBG_ON(A, 2)) mbar_wait(&S.full_bar[stage], par);
-        const int ro0 = R0[stage * kKS], ro1 = R0[stage * kKS + 1];
+        int ro0, ro1;
+        float fy0 = 0.0f, fy1 = 0.0f;
+        if (MODE == 3) {                       // du = 1: top row and weight of the whole tile from the FP64 origin
+            const double v0 = T.vrel[0], v1 = T.vrel[1], f0 = floor(v0), f1 = floor(v1);
+            ro0 = (int)f0; ro1 = (int)f1; fy0 = (float)(v0 - f0); fy1 = (float)(v1 - f1);
+        } else { ro0 = R0[stage * kKS]; ro1 = R0[stage * kKS + 1]; }
         u64 ref;
         {
             const u64 a0 = uf0 + colW, a1 = a0 + (u64)NT * du64;
@@ -326,7 +369,8 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
                 const uint32_t rowb = tile_s + (uint32_t)ro0 * pb;
                 const uint32_t t0 = rowb + (uint32_t)(U0 >> 32) * 4u, t1 = rowb + (uint32_t)(U1 >> 32) * 4u;
                 const uint32_t wt_s = w_s + (uint32_t)(stage * kKS + 0) * (kTR * 16);
-                if (MODE == 2) t2_march_quad<0>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 0) * 4));
+                if (MODE == 3) t2_march_unit<0>(acc, t0, t1, fx, ref, 1.0f - fy0, fy0);
+                else if (MODE == 2) t2_march_quad<0>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 0) * 4));
                 else if (MODE == 1) t2_march_any<0>(acc, t0, t1, pb, fx, ref, wt_s);
                 else t2_march<0>(acc, t0, t1, fx, ref, wt_s);
             }
@@ -336,7 +380,8 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
                 const uint32_t rowb = tile_s + (uint32_t)ro1 * pb;
                 const uint32_t t0 = rowb + (uint32_t)(U0 >> 32) * 4u, t1 = rowb + (uint32_t)(U1 >> 32) * 4u;
                 const uint32_t wt_s = w_s + (uint32_t)(stage * kKS + 1) * (kTR * 16);
-                if (MODE == 2) t2_march_quad<kTR>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 1) * 4));
+                if (MODE == 3) t2_march_unit<kTR>(acc, t0, t1, fx, ref, 1.0f - fy1, fy1);
+                else if (MODE == 2) t2_march_quad<kTR>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 1) * 4));
                 else if (MODE == 1) t2_march_any<kTR>(acc, t0, t1, pb, fx, ref, wt_s);
                 else t2_march<kTR>(acc, t0, t1, fx, ref, wt_s);
             }

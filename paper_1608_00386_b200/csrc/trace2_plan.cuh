@@ -13,15 +13,17 @@ namespace ao {
 constexpr int kFusedThreads = 128;
 constexpr int kTileCols = 2 * kFusedThreads;
 
-struct Tile2Plan { bool ok; int pitch, rows, ns; size_t smem; int anydu, quad; };
+struct Tile2Plan { bool ok; int pitch, rows, ns; size_t smem; int anydu, quad, unit; };
 
 // Staging plan of the two-step tiled ray-trace for the sources `src` (all active layers): the union box of a
 // 16 x 256 tile over two consecutive steps must fit a shared-memory stage.  Layers with 1/2 <= du <= 1 (screen
 // pixels per output sample) take the three-term row march; if any layer is outside, the two-row march runs.  `min_bytes`: floor on the stage region (the exchange buffer of k_fused aliases it).
-inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, double dt, size_t min_bytes)
+inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, double dt, size_t min_bytes,
+                             size_t budget = 55 * 1024 + 512)
 {
-    Tile2Plan pl = {false, 0, 0, 0, 0, 0, 0};
+    Tile2Plan pl = {false, 0, 0, 0, 0, 0, 0, 0};
     double du_max = 0.0;
+    bool all_unit = true;
     double ext_x = 0.0, ext_y = 0.0;                               // box extent beyond the taps, screen pixels
     int s_min = 1 << 30;
     bool any = false;
@@ -34,6 +36,7 @@ inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, 
             if (!(du > 0.0) || du > 8.0) return pl;               // absurd sampling ratio: not this path
             if (du < 0.5 || du > 1.0) pl.anydu = 1;                // outside the three-term march: two-row march
             if (du > du_max) du_max = du;
+            if (du != 1.0) all_unit = false;
             if (lp.S % 4 != 0 || ((uintptr_t)lp.screen & 15) != 0) return pl;   // 16-byte aligned rows for the bulk copies
             const double shx = fabs(lp.wx * dt * lp.inv_pitch) * (kKS - 1), shy = fabs(lp.wy * dt * lp.inv_pitch) * (kKS - 1);
             ext_x = std::max(ext_x, (kTileCols - 1) * du + shx);
@@ -46,12 +49,12 @@ inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, 
     if (!(ext_x < 4096.0 && ext_y < 4096.0)) return pl;            // absurd wind shift per step: not this path
     pl.pitch = (((int)ceil(ext_x) + 8) + 3) & ~3;                  // + alignment (3), right tap, rounding slack
     pl.quad = (pl.anydu && du_max <= 0.66) ? 1 : 0;                // every layer has du <= 2/3: groups of four rows
+    if (any && all_unit && pl.pitch <= kUnitPitch) { pl.unit = 1; pl.pitch = kUnitPitch; }   // du = 1: table-free march
     pl.rows = (int)ceil(ext_y) + 3 + 1 + (pl.quad ? 2 : 0);        // box rows + one pad row (+ the quad march's fourth row)
     if (s_min < pl.pitch || s_min < pl.rows) return pl;            // a box row may wrap the screen edge once only
     const size_t stage = (size_t)pl.rows * pl.pitch * sizeof(float);
     const size_t sched = trace2_sched_bytes((int)g->layers.size());
-    // 4 CTAs per SM: <= ~55 KB of shared memory each; as many stages (<= 4) as fit, at least 2
-    const size_t budget = 55 * 1024 + 512;
+    // fused kernel: 4 CTAs per SM, <= ~55 KB of shared memory each; as many stages (<= 4) as fit the budget, at least 2
     pl.ns = 2;
     while (pl.ns < kT2MaxStages && (pl.ns + 1) * stage + sched + 128 + 256 <= budget) ++pl.ns;
 #ifdef AO_PROFILE_SWITCHES      // profiling builds only: override the stage count
