@@ -86,6 +86,7 @@ static void destroy(ao_geometry* g)
     for (auto& w : g->wfs) {
         cudaFree(w.d_amp); cudaFree(w.d_valid); cudaFree(w.d_w2m); cudaFree(w.d_tw); cudaFree(w.d_twf); cudaFree(w.d_pre); cudaFree(w.fused_items);
         free_sodium(w);
+        cudaFree(w.d_tmaps);
         free_group(w.grp);
     }
     free_group(g->all); free_group(g->sci);
@@ -384,6 +385,7 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
             int* d = nullptr;
             if ((e = upload(&d, items.data(), items.size())) != cudaSuccess) return bail("fused items upload");
             w.fused_items = d;
+            if (n_layers > 0 && (e = cudaMalloc((void**)&w.d_tmaps, (size_t)n_layers * (128 + sizeof(int2)))) != cudaSuccess) return bail("tensor map table");
         }
         if (w.M <= 64) {      // direct-DFT table of k_sh_generic (M = 64 uses it for extended beacons only)
             std::vector<float2> t(2 * w.M);

@@ -75,6 +75,9 @@ struct WfsH {
     float2* d_twf = nullptr;        // exp(-2 pi i k / M), k < M           (big path, Stockham passes)
     float2* d_pre = nullptr;        // pre-twiddle exp(+i pi (M-1) a / M), a < n  (big path)
     SodiumP na;                     // extended beacon (device pointers owned by the handle), n_z = 0: none
+    unsigned char* d_tmaps = nullptr;   // CUtensorMap[n_layers] of the fused kernel's staged boxes (device), see k_fused.cu
+    int tm_pitch = 0, tm_rows = 0;      // plan the maps were encoded for (0: not encoded yet)
+    double tm_dt = 0.0;
     void* fused_items = nullptr;    // device WorkItem[]: runs of <= fused_G adjacent valid subapertures
     int n_fused_items = 0, fused_G = 0, fused_R2 = 0;
     Group grp;

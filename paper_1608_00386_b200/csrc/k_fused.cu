@@ -25,6 +25,9 @@
 #include <type_traits>
 #include <vector>
 
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
 #include "fft_reg.cuh"
 #include "trace2.cuh"
 #include "trace2_plan.cuh"
@@ -259,6 +262,64 @@ void fused_tile_shape(int M, int* G, int* R2)
 
 static size_t fused_xch_bytes(int M) { return M == 32 ? FusedCfg<32>::XCH_BYTES : FusedCfg<16>::XCH_BYTES; }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda); NULL if unavailable.
+static PFN_cuTensorMapEncodeTiled tensor_map_encoder()
+{
+    static PFN_cuTensorMapEncodeTiled fn = []() -> PFN_cuTensorMapEncodeTiled {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess) { cudaGetLastError(); return nullptr; }
+        return (PFN_cuTensorMapEncodeTiled)p;
+    }();
+    return fn;
+}
+
+// One tensor map per layer over the borrowed screen [S][S], each with its OWN box {pitch_l, rows_l} (the extent of a tile
+// on that layer: du and the wind shift differ per layer, so a common box would overfetch): the staged box of a tile is
+// then a single cp.async.bulk.tensor.2d (UTMALDG) instead of one bulk copy per row.  Encoded once per (plan, dt), cached.
+static cudaError_t ensure_tensor_maps(ao_geometry* g, WfsH& w, const Tile2Plan& pl, double dt, cudaStream_t st)
+{
+    if (w.tm_pitch == pl.pitch && w.tm_rows == pl.rows && w.tm_dt == dt) return cudaSuccess;
+    PFN_cuTensorMapEncodeTiled enc = tensor_map_encoder();
+    if (!enc || !w.d_tmaps) return cudaErrorNotSupported;
+    const size_t nl = g->layers.size();
+    std::vector<unsigned char> buf(nl * (sizeof(CUtensorMap) + sizeof(int2)));
+    CUtensorMap* maps = reinterpret_cast<CUtensorMap*>(buf.data());
+    int2* boxes = reinterpret_cast<int2*>(buf.data() + nl * sizeof(CUtensorMap));
+    for (size_t l = 0; l < nl; ++l) {
+        const LayerP& lp = g->layers[l];
+        // this layer's own box: the extent of a tile over the two paired steps, as in plan_tiles2 but per layer
+        double ext_x = 0.0, ext_y = 0.0;
+        for (int s : w.grp.src) {
+            const SourceP& sp = g->sources[s];
+            if (!(lp.height < sp.H)) continue;
+            double du = (1.0 - lp.height * sp.inv_H) * sp.d * lp.inv_pitch;
+            if (fabs(du - 1.0) < 1e-9) du = 1.0;
+            ext_x = std::max(ext_x, (kTileCols - 1) * du + fabs(lp.wx * dt * lp.inv_pitch) * (kKS - 1));
+            ext_y = std::max(ext_y, (kTR - 1) * du + fabs(lp.wy * dt * lp.inv_pitch) * (kKS - 1));
+        }
+        int pt = std::min(pl.pitch, (((int)ceil(ext_x) + 8) + 7) & ~7);
+        int rw = std::min(pl.rows, (int)ceil(ext_y) + 3 + (pl.quad ? 2 : 0));
+        if (pt < 8) pt = 8;
+        if (rw < 1) rw = 1;
+        boxes[l] = make_int2(pt, rw);
+        const cuuint64_t dims[2] = {(cuuint64_t)lp.S, (cuuint64_t)lp.S};
+        const cuuint64_t strides[1] = {(cuuint64_t)lp.S * sizeof(float)};
+        const cuuint32_t box[2] = {(cuuint32_t)pt, (cuuint32_t)rw};
+        const cuuint32_t estr[2] = {1, 1};
+        if (lp.S < pt || lp.S < rw ||
+            enc(&maps[l], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)lp.screen, dims, strides, box, estr,
+                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return cudaErrorNotSupported;
+    }
+    static_assert(sizeof(CUtensorMap) == 128, "tensor maps are indexed by 128 bytes in trace2.cuh");
+    cudaError_t e = cudaMemcpyAsync(w.d_tmaps, buf.data(), buf.size(), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) { w.tm_pitch = pl.pitch; w.tm_rows = pl.rows; w.tm_dt = dt; }
+    return e;
+}
+
 bool fused_supported(const ao_geometry* g, const WfsH& w, double dt)
 {
     if (!(w.M == 16 || w.M == 32) || w.n * 2 != w.M || w.P != 8 || w.beta * w.P != w.M) return false;
@@ -305,7 +366,11 @@ cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_ste
                          const NoiseP& noise, float* images, float* slopes, cudaStream_t st)
 {
     if (!fused_supported(g, w, dt)) return cudaErrorNotSupported;
-    const Tile2Plan pl = plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M));
+    Tile2Plan pl = plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M), 55 * 1024 + 512, w.d_tmaps != nullptr);
+    if (pl.tma && (!pl.ok || ensure_tensor_maps(g, const_cast<WfsH&>(w), pl, dt, st) != cudaSuccess)) {
+        cudaGetLastError();
+        pl = plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M));      // per-row bulk copies
+    }
     const size_t n_sel = w.grp.src.size(), nsa = (size_t)w.n_sub * w.n_sub;
     cudaError_t e;
     // invalid subapertures are never scheduled: zero-fill the outputs first
@@ -313,6 +378,7 @@ cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_ste
     if (slopes && (e = cudaMemsetAsync(slopes, 0, sizeof(float) * n_steps * n_sel * 2 * nsa, st)) != cudaSuccess) return e;
     FusedArgs a;
     a.T = make_trace2_args(g, pl, step0, dt);
+    if (pl.tma) a.T.tmaps = w.d_tmaps;
     a.sel = w.grp.d_src; a.n_sel = (int)n_sel;
     a.items = (const WorkItem*)w.fused_items; a.n_items = w.n_fused_items; a.n_steps = n_steps;
     a.amp = w.d_amp; a.valid = w.d_valid; a.n_sub = w.n_sub;

@@ -77,6 +77,15 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+// 2-D tensor-map TMA load (cp.async.bulk.tensor, SASS UTMALDG): the box {boxDim0, boxDim1} of the map at element
+// coordinates (c0 = column, c1 = row) into shared memory, row pitch boxDim0; out-of-bounds elements are zero-filled and
+// still counted in the transaction bytes.  `tmap`: CUtensorMap in global memory (written by the host before the launch).
+__device__ __forceinline__ void tma_load_2d(void* dst, const void* tmap, int c0, int c1, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst)), "l"(tmap), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
+
 // ---- shared-memory loads by 32-bit shared address ----
 __device__ __forceinline__ float lds_f32(uint32_t addr)
 {

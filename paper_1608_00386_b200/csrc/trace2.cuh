@@ -45,6 +45,7 @@ struct Trace2Args {
     int pitch;            // staged row pitch in floats (multiple of 4)
     int rows;             // staged rows allocated per stage (box rows + 1 prefetch pad row)
     int ns;               // stages in flight
+    const unsigned char* tmaps;   // per-layer CUtensorMap[n_layers] (128 bytes each), then int2 box {pitch_l, rows_l}[n_layers]; or NULL
 #ifdef AO_PROFILE_SWITCHES
     int dbg;              // profiling builds only (AO_DBG): 1 = skip the row march, 2 = skip staging, 4 = skip image formation
 #endif
@@ -66,6 +67,8 @@ struct __align__(16) LayerT {
     unsigned duf;         // frac(du) 2^32
     int du_hi;            // floor(du)
     int lay;              // layer index
+    int tm;               // 1: the box does not wrap the screen edge and a tensor map exists: one TMA tensor copy
+    int pitch, box_rows;  // shared-memory row pitch of this layer's box (the map's own box with a tensor copy) and its rows
     double du;            // screen pixels per output sample
     double vrel[kKS];     // row coordinate of tile row 0 relative to box row 0
     u64 uf[kKS];          // (column coordinate of tile column 0 - box column 0) 2^32
@@ -251,6 +254,11 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         long long cw = cmin % lp.S; if (cw < 0) cw += lp.S;
         long long rw = rmin % lp.S; if (rw < 0) rw += lp.S;
         T.scr = lp.screen; T.S = lp.S; T.cw = (int)cw; T.rw = (int)rw; T.wt = wt; T.rt = rt;
+        T.tm = 0; T.pitch = pitch; T.box_rows = 0;
+        if (A.tmaps != nullptr) {                                  // this layer's own box {pitch_l, rows_l}: no overfetch
+            const int2 bx = reinterpret_cast<const int2*>(A.tmaps + (size_t)A.n_layers * 128)[T.lay];
+            if (wt <= bx.x && rt <= bx.y && cw + wt <= lp.S && rw + rt <= lp.S) { T.tm = 1; T.pitch = bx.x; T.box_rows = bx.y; }
+        }
         T.du = du; T.du_hi = (int)floor(du);
         const unsigned long long f = __double2ull_rn((du - (double)T.du_hi) * 4294967296.0);
         T.duf = f > 0xffffffffull ? 0xffffffffu : (unsigned)f;
@@ -265,7 +273,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
     // producer (one warp): row table + TMA bulk row copies of active layer `a` into `stage`
     auto issue = [&](int a, int stage) {
         const LayerT& T = L[a];
-        const int wt = T.wt, rt = T.rt, Sn = T.S, cw = T.cw, rw = T.rw;
+        const int wt = T.wt, rt = T.rt, Sn = T.S, cw = T.cw, rw = T.rw, pitch = T.pitch;
         const float* scr = T.scr;
         uint64_t* bar = &S.full_bar[stage];
         float* dst = tiles + (size_t)stage * tile_floats;
@@ -305,6 +313,13 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         }
         __syncwarp();
         if (AO_DBG_ON(A, 2)) return;
+        if (T.tm) {                                        // whole box in one tensor copy (rows beyond the screen: zero fill)
+            if (lane == 0) {
+                mbar_expect_tx(bar, (uint32_t)(T.pitch * T.box_rows) * 4u);
+                tma_load_2d(dst, A.tmaps + (size_t)T.lay * 128, cw, rw, bar);
+            }
+            return;
+        }
         if (lane == 0) mbar_expect_tx(bar, (uint32_t)(rt * wt) * 4u);
         __syncwarp();
         const int first = (cw + wt <= Sn) ? wt : Sn - cw;                     // floats before the periodic wrap
@@ -324,7 +339,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
     __syncthreads();
 
     const uint32_t tiles_s = smem_u32(tiles), w_s = smem_u32(Wt);
-    const uint32_t pb = (uint32_t)pitch * 4u, tile_bytes = (uint32_t)tile_floats * 4u;
+    const uint32_t tile_bytes = (uint32_t)tile_floats * 4u;
     int stage = 0;
     uint32_t par = 0;                          // stage and parity of layer a
     // Refill lag: at iteration a the producer refills the stage of layer a - lag with layer a - lag + ns.  With
@@ -341,6 +356,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             issue(l + ns, l - m * ns);
         }
         const LayerT& T = L[a];
+        const uint32_t pb = (uint32_t)T.pitch * 4u;
         const u64 du64 = ((u64)(unsigned)T.du_hi << 32) | (u64)T.duf;
         const u64 uf0 = T.uf[0], uf1 = T.uf[1];
         const uint32_t tile_s = tiles_s + (uint32_t)stage * tile_bytes;

@@ -13,15 +13,15 @@ namespace ao {
 constexpr int kFusedThreads = 128;
 constexpr int kTileCols = 2 * kFusedThreads;
 
-struct Tile2Plan { bool ok; int pitch, rows, ns; size_t smem; int anydu, quad, unit; };
+struct Tile2Plan { bool ok; int pitch, rows, ns; size_t smem; int anydu, quad, unit, tma; };
 
 // Staging plan of the two-step tiled ray-trace for the sources `src` (all active layers): the union box of a
 // 16 x 256 tile over two consecutive steps must fit a shared-memory stage.  Layers with 1/2 <= du <= 1 (screen
 // pixels per output sample) take the three-term row march; if any layer is outside, the two-row march runs.  `min_bytes`: floor on the stage region (the exchange buffer of k_fused aliases it).
 inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, double dt, size_t min_bytes,
-                             size_t budget = 55 * 1024 + 512)
+                             size_t budget = 55 * 1024 + 512, bool want_tma = false)
 {
-    Tile2Plan pl = {false, 0, 0, 0, 0, 0, 0, 0};
+    Tile2Plan pl = {false, 0, 0, 0, 0, 0, 0, 0, 0};
     double du_max = 0.0;
     bool all_unit = true;
     double ext_x = 0.0, ext_y = 0.0;                               // box extent beyond the taps, screen pixels
@@ -51,6 +51,11 @@ inline Tile2Plan plan_tiles2(const ao_geometry* g, const std::vector<int>& src, 
     pl.quad = (pl.anydu && du_max <= 0.66) ? 1 : 0;                // every layer has du <= 2/3: groups of four rows
     if (any && all_unit && pl.pitch <= kUnitPitch) { pl.unit = 1; pl.pitch = kUnitPitch; }   // du = 1: table-free march
     pl.rows = (int)ceil(ext_y) + 3 + 1 + (pl.quad ? 2 : 0);        // box rows + one pad row (+ the quad march's fourth row)
+    if (want_tma && any && !pl.unit) {
+        // tensor-map copies: box {pitch, rows} <= 256 x 256, stages 128-byte aligned (rows * pitch a multiple of 32 floats)
+        const int pt = (pl.pitch + 7) & ~7, rw = (pl.rows + 3) & ~3;
+        if (pt <= 256 && rw <= 256) { pl.tma = 1; pl.pitch = pt; pl.rows = rw; }
+    }
     if (s_min < pl.pitch || s_min < pl.rows) return pl;            // a box row may wrap the screen edge once only
     const size_t stage = (size_t)pl.rows * pl.pitch * sizeof(float);
     const size_t sched = trace2_sched_bytes((int)g->layers.size());
@@ -72,6 +77,7 @@ inline Trace2Args make_trace2_args(const ao_geometry* g, const Tile2Plan& pl, in
     Trace2Args t;
     t.layers = g->d_layers; t.n_layers = (int)g->layers.size(); t.srcs = g->d_sources;
     t.step0 = (long long)step0; t.dt = dt; t.pitch = pl.pitch; t.rows = pl.rows; t.ns = pl.ns;
+    t.tmaps = nullptr;
 #ifdef AO_PROFILE_SWITCHES      // profiling builds only (AO_BUILD_PROFILE=1): switch parts of the kernel off, results are wrong
     { const char* ev = getenv("AO_DBG"); t.dbg = ev ? atoi(ev) : 0; }
 #endif
