@@ -93,6 +93,7 @@ k_sh_reg(const ShRegArgs A)
     }
     __syncwarp();
     float s = 0.0f, mx = 0.0f, my = 0.0f;
+    const float hP = 0.5f * (float)(P - 1);
     if (item_on) {
         float* img = A.images ? A.images + (size_t)item * (P * P) : nullptr;
         for (int px = b; px < P * P; px += n) {                 // detector pixel = sum of its beta rows
@@ -105,16 +106,28 @@ k_sh_reg(const ShRegArgs A)
             if (!active) v = 0.0f;
             if (img) img[px] = v;
             pix[px] = v;
+            s += v; mx = fmaf((float)c - hP, v, mx); my = fmaf((float)r - hP, v, my);
         }
     }
-    __syncwarp();
-    if (item_on && b == 0 && A.slopes) {                        // centre of gravity in pixel order (36 .. 64 terms)
-        const float h = 0.5f * (float)(P - 1);
-        for (int px = 0; px < P * P; ++px) {
-            const int r = px / P, c = px - r * P;
-            const float v = pix[px];
-            s += v; mx = fmaf((float)c - h, v, mx); my = fmaf((float)r - h, v, my);
+    if constexpr ((n & (n - 1)) == 0) {                          // centre of gravity: butterfly over the group's n lanes
+#pragma unroll
+        for (int o = n / 2; o >= 1; o >>= 1) {
+            s += __shfl_xor_sync(0xffffffffu, s, o);
+            mx += __shfl_xor_sync(0xffffffffu, mx, o);
+            my += __shfl_xor_sync(0xffffffffu, my, o);
         }
+    } else {                                                     // n = 12: the group's first lane sums the pixels in order
+        __syncwarp();
+        if (item_on && b == 0) {
+            s = 0.0f; mx = 0.0f; my = 0.0f;
+            for (int px = 0; px < P * P; ++px) {
+                const int r = px / P, c = px - r * P;
+                const float v = pix[px];
+                s += v; mx = fmaf((float)c - hP, v, mx); my = fmaf((float)r - hP, v, my);
+            }
+        }
+    }
+    if (item_on && b == 0 && A.slopes) {
         const bool ok = active && fabsf(s) >= 1e-12f;
         A.slopes[((size_t)set * 2 + 0) * A.nsa + sa] = ok ? mx / s : 0.0f;
         A.slopes[((size_t)set * 2 + 1) * A.nsa + sa] = ok ? my / s : 0.0f;
