@@ -179,7 +179,7 @@ static int run_wfs(ao_geometry* g, int wi, const float* phase_dev, int64_t step0
     WfsH& w = g->wfs[wi];
     const size_t n_sel = w.grp.src.size(), nsa = (size_t)w.n_sub * w.n_sub, PP = (size_t)w.P * w.P;
     if (n_sel == 0) return AO_OK;
-    if (!phase_dev && !w.big) {                       // hot path: one fused kernel, no phase in HBM, no workspace
+    if (!phase_dev && (!w.big || w.M == 64)) {        // hot path: one fused kernel, no phase in HBM, no workspace
         if (fused_supported(g, w, dt)) {
             AO_CUDA(launch_fused(g, w, step0, n_steps, dt, make_noise(noise), images, slopes, st), "fused");
             return AO_OK;
@@ -556,7 +556,7 @@ static int forward_chunk(ao_geometry* g, int64_t step0, int n_steps, double dt_s
     for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
         const WfsH& w = g->wfs[wi];
         if (!slopes || !slopes[wi] || w.grp.src.empty()) continue;
-        const bool ws_free = !w.big && fused_supported(g, w, dt_s);
+        const bool ws_free = (!w.big || w.M == 64) && fused_supported(g, w, dt_s);
         on_side[wi] = ws_free ? 0 : 1;
         (ws_free ? any_free : any_ws) = true;
     }

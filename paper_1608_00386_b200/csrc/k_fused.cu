@@ -251,16 +251,151 @@ k_fused(const FusedArgs A)
 }
 
 // ------------------------------------------------------------------------------------------------
+// k_fused64: the same fusion for M = 64 (n = 32 samples per subaperture, 8 x 8 pixels of 8 x 8 FFT pixels; c4's largest
+// sweep point).  A work item is one subaperture row of up to 8 adjacent subapertures = 32 x 256 samples, for two steps.
+// The 16-row tile of trace2.cuh is marched twice: the top half's sums go to a shared-memory stash (each thread reads
+// back only what it wrote), the bottom half stays in registers.  The two halves carry different warp-uniform piston
+// references; their FP64 difference is added to the top half so that a subaperture has ONE piston (which |FFT|^2 does
+// not see).  Image formation: one warp per subaperture and round (step, column half): thread b holds column b
+// (32 samples), two 32-point FFTs in registers (dft_half_padded<64>), transpose through shared memory, rows b and
+// b + 32, |.|^2, 8 x 8 binning (8 columns in registers, 8 rows through shared memory), noise, centre of gravity.
+constexpr int kF64Stash = kKS * kTR * kTileCols * (int)sizeof(float);                 // 32 KB
+constexpr int kF64XP = 33;                                                              // transpose pitch, float2
+constexpr int kF64Sub = 64 * kF64XP * (int)sizeof(float2) + (64 * 8 + 64) * (int)sizeof(float);   // per warp: T[64][33], row bins, pixels
+constexpr size_t kF64Xch = 4 * (size_t)kF64Sub;
+
+template <int MODE, bool NOISE>
+__global__ void __launch_bounds__(kFusedThreads, 2)
+k_fused64(const FusedArgs A, const unsigned stash_off)
+{
+    constexpr int M = 64, n = 32, P = 8, BETA = 8, NT = kFusedThreads;
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ Trace2Shared S;
+    const int tid = threadIdx.x, warp = tid >> 5, b = tid & 31;
+    const int kp = (int)(blockIdx.x % (unsigned)A.n_pairs);
+    const unsigned rest = blockIdx.x / (unsigned)A.n_pairs;
+    const WorkItem it = A.items[rest % (unsigned)A.n_items];
+    const int si = (int)(rest / (unsigned)A.n_items);
+    const int src_index = A.sel[si];
+    const SourceP sp = A.T.srcs[src_index];
+    const int N = A.n_sub * n, nsa = A.n_sub * A.n_sub;
+    float* stash = reinterpret_cast<float*>(smem + stash_off);     // [step][row < 16][column < 256]
+
+    u64 acc[kKS * kTR];
+    double rs_top[2], rs_bot[2];
+    trace2_tile<NT, true, MODE>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, rs_top);
+#pragma unroll
+    for (int i = 0; i < kKS * kTR; ++i) {
+        const float2 f = unpack2(acc[i]);
+        stash[i * kTileCols + tid] = f.x;
+        stash[i * kTileCols + NT + tid] = f.y;
+    }
+    __syncthreads();                                       // every warp has left the first march: barriers and stages are re-armed
+    trace2_tile<NT, true, MODE>(A.T, sp, S, smem, it.q0 * n, it.p * n + kTR, A.T.step0 + 2 * kp, acc, rs_bot);
+    __syncthreads();                                       // stages are dead: shared memory becomes the exchange buffer
+    const float dref[2] = {(float)(rs_top[0] - rs_bot[0]), (float)(rs_top[1] - rs_bot[1])};
+
+    unsigned char* wbuf = smem + (size_t)warp * kF64Sub;
+    float2* xs = reinterpret_cast<float2*>(wbuf);                              // T[k][b]
+    float* rb = reinterpret_cast<float*>(wbuf + 64 * kF64XP * sizeof(float2));   // row bins [64][8]
+    float* pix = rb + 64 * 8;
+    const float scale = (float)sp.scale;
+    const float* mp = sp.map;
+    const int p = it.p;
+#pragma unroll 1
+    for (int rd = 0; rd < 4; ++rd) {
+        const int s2 = rd >> 1, c = rd & 1;                // step in pair, column half: subaperture c * 4 + warp of the item
+        const int k = 2 * kp + s2;
+        const size_t set = (size_t)k * A.n_sel + si;
+        const int gs = c * 4 + warp, q = it.q0 + gs;
+        const bool inb = gs < it.cnt && k < A.n_steps;
+        const int sa = inb ? p * A.n_sub + q : 0;
+        const bool active = inb && A.valid[sa] != 0;      // warp-uniform
+        if (!active) continue;
+        __syncwarp();                                      // the previous round has finished reading xs
+        {
+            float2 e[n];
+            const float* ap = A.amp + (size_t)(p * n) * N + (size_t)q * n + b;
+            const float* st = stash + (size_t)(s2 * kTR) * kTileCols + c * NT + tid;
+#pragma unroll
+            for (int i = 0; i < n; ++i) {
+                float ph;
+                if (i < kTR) ph = st[i * kTileCols] + dref[c];
+                else {
+                    const float2 f = unpack2(s2 ? acc[kTR + i - kTR] : acc[i - kTR]);
+                    ph = c ? f.y : f.x;
+                }
+                ph *= scale;
+                if (mp) ph += __ldg(mp + (size_t)(p * n + i) * N + (size_t)q * n + b);
+                const float Am = __ldg(ap + (size_t)i * N);
+                float sn, co;
+                sincos_reduced(ph, &sn, &co);
+                e[i] = make_float2(Am * co, Am * sn);
+            }
+            dft_half_padded<M>(e, [&](auto ki, const float2 v) {
+                constexpr int kk = decltype(ki)::value;
+                xs[kk * kF64XP + b] = v;
+            });
+        }
+        __syncwarp();
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {                   // rows b and b + 32
+            const int kr = b + hh * n;
+            float2 rrow[n];
+#pragma unroll
+            for (int i = 0; i < n; ++i) rrow[i] = xs[kr * kF64XP + i];
+            float bins[P];
+#pragma unroll
+            for (int i = 0; i < P; ++i) bins[i] = 0.0f;
+            dft_half_padded<M>(rrow, [&](auto mi, const float2 v) {
+                constexpr int m = decltype(mi)::value;
+                bins[m / BETA] = fmaf(v.x, v.x, fmaf(v.y, v.y, bins[m / BETA]));
+            });
+#pragma unroll
+            for (int i = 0; i < P; ++i) rb[kr * P + i] = bins[i];
+        }
+        __syncwarp();
+        float s = 0.0f, mx = 0.0f, my = 0.0f;
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {                      // pixels b and b + 32: sum of their 8 rows
+            const int px = b + t * 32, r = px >> 3, col = px & 7;
+            float v = 0.0f;
+#pragma unroll
+            for (int y = 0; y < BETA; ++y) v += rb[(r * BETA + y) * P + col];
+            v *= A.norm;
+            if (NOISE) v = noisy_pixel(v, A.nz, (uint32_t)px, (uint32_t)sa, (uint32_t)src_index, (uint32_t)(A.T.step0 + k));
+            if (A.images) A.images[(set * nsa + sa) * (P * P) + px] = v;
+            s += v;
+            mx = fmaf((float)col - 0.5f * (P - 1), v, mx);
+            my = fmaf((float)r - 0.5f * (P - 1), v, my);
+        }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) {
+            s += __shfl_xor_sync(0xffffffffu, s, o);
+            mx += __shfl_xor_sync(0xffffffffu, mx, o);
+            my += __shfl_xor_sync(0xffffffffu, my, o);
+        }
+        if (A.slopes && b == 0) {
+            const bool ok = fabsf(s) >= 1e-12f;
+            A.slopes[(set * 2 + 0) * nsa + sa] = ok ? mx / s : 0.0f;
+            A.slopes[(set * 2 + 1) * nsa + sa] = ok ? my / s : 0.0f;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // host side
 // Tile shape of the fused kernel per FFT size: G subapertures wide, R2 subaperture rows tall.
 void fused_tile_shape(int M, int* G, int* R2)
 {
     if (M == 32) { *G = FusedCfg<32>::G; *R2 = FusedCfg<32>::R2; }
     else if (M == 16) { *G = FusedCfg<16>::G; *R2 = FusedCfg<16>::R2; }
+    else if (M == 64) { *G = kTileCols / 32; *R2 = 1; }            // k_fused64: one subaperture row of 8 per work item
     else { *G = 0; *R2 = 0; }
 }
 
-static size_t fused_xch_bytes(int M) { return M == 32 ? FusedCfg<32>::XCH_BYTES : FusedCfg<16>::XCH_BYTES; }
+static size_t fused_xch_bytes(int M) { return M == 64 ? kF64Xch : M == 32 ? FusedCfg<32>::XCH_BYTES : FusedCfg<16>::XCH_BYTES; }
+static size_t fused_budget(int M) { return M == 64 ? 72 * 1024 : 55 * 1024 + 512; }     // M = 64: 2 CTAs per SM
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda); NULL if unavailable.
 static PFN_cuTensorMapEncodeTiled tensor_map_encoder()
@@ -322,9 +457,11 @@ static cudaError_t ensure_tensor_maps(ao_geometry* g, WfsH& w, const Tile2Plan& 
 
 bool fused_supported(const ao_geometry* g, const WfsH& w, double dt)
 {
-    if (!(w.M == 16 || w.M == 32) || w.n * 2 != w.M || w.P != 8 || w.beta * w.P != w.M) return false;
+    if (!(w.M == 16 || w.M == 32 || w.M == 64) || w.n * 2 != w.M || w.P != 8 || w.beta * w.P != w.M) return false;
     if (w.fused_items == nullptr || w.n_fused_items == 0) return false;
-    return plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M)).ok;
+    if (w.M == 64 && w.na.n_z > 0) return false;           // extended beacons at M = 64 run k_sh_generic
+    const Tile2Plan pl = plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M), fused_budget(w.M));
+    return pl.ok && (w.M != 64 || pl.smem + 128 + kF64Stash <= 113 * 1024);
 }
 
 template <int M>
@@ -362,14 +499,43 @@ static cudaError_t launch_fused_variant(ao_geometry* g, const WfsH& w, FusedArgs
     return cudaSuccess;
 }
 
+static cudaError_t launch_fused64(ao_geometry* g, const WfsH& w, FusedArgs a, const Tile2Plan& pl, int n_steps, cudaStream_t st)
+{
+    void (*kern)(const FusedArgs, const unsigned);
+    const int mode = pl.quad ? 2 : (pl.anydu ? 1 : 0);
+    if (a.nz.on) kern = mode == 2 ? k_fused64<2, true> : mode == 1 ? k_fused64<1, true> : k_fused64<0, true>;
+    else kern = mode == 2 ? k_fused64<2, false> : mode == 1 ? k_fused64<1, false> : k_fused64<0, false>;
+    const unsigned stash_off = (unsigned)((pl.smem + 127) & ~(size_t)127);
+    const size_t smem = (size_t)stash_off + kF64Stash;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const size_t nsa = (size_t)w.n_sub * w.n_sub;
+    const long long per_pair = (long long)a.n_items * a.n_sel;
+    int max_steps = (int)std::max<long long>(2, 2 * (0x7fffffffLL / per_pair));
+    max_steps &= ~1;
+    const int64_t step0 = a.T.step0;
+    for (int k0 = 0; k0 < n_steps; k0 += max_steps) {
+        const int ks = n_steps - k0 < max_steps ? n_steps - k0 : max_steps;
+        FusedArgs b = a;
+        b.T.step0 = step0 + k0; b.n_steps = ks; b.n_pairs = (ks + kKS - 1) / kKS;
+        const size_t set0 = (size_t)k0 * a.n_sel;
+        if (a.images) b.images = a.images + set0 * nsa * w.P * w.P;
+        if (a.slopes) b.slopes = a.slopes + set0 * 2 * nsa;
+        kern<<<(unsigned)(per_pair * b.n_pairs), kFusedThreads, smem, st>>>(b, stash_off);
+        g->launches++;
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
 cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_steps, double dt,
                          const NoiseP& noise, float* images, float* slopes, cudaStream_t st)
 {
     if (!fused_supported(g, w, dt)) return cudaErrorNotSupported;
-    Tile2Plan pl = plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M), 55 * 1024 + 512, w.d_tmaps != nullptr);
+    Tile2Plan pl = plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M), fused_budget(w.M), w.d_tmaps != nullptr);
     if (pl.tma && (!pl.ok || ensure_tensor_maps(g, const_cast<WfsH&>(w), pl, dt, st) != cudaSuccess)) {
         cudaGetLastError();
-        pl = plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M));      // per-row bulk copies
+        pl = plan_tiles2(g, w.grp.src, dt, fused_xch_bytes(w.M), fused_budget(w.M));      // per-row bulk copies
     }
     const size_t n_sel = w.grp.src.size(), nsa = (size_t)w.n_sub * w.n_sub;
     cudaError_t e;
@@ -384,6 +550,7 @@ cudaError_t launch_fused(ao_geometry* g, const WfsH& w, int64_t step0, int n_ste
     a.amp = w.d_amp; a.valid = w.d_valid; a.n_sub = w.n_sub;
     a.norm = (float)(1.0 / ((double)w.M * w.M * (double)w.n * w.n));
     a.nz = noise; a.images = images; a.slopes = slopes; a.na = w.na;
+    if (w.M == 64) return launch_fused64(g, w, a, pl, n_steps, st);
     if (w.M == 32) return launch_fused_variant<32>(g, w, a, pl, n_steps, st);
     return launch_fused_variant<16>(g, w, a, pl, n_steps, st);
 }
