@@ -29,6 +29,9 @@ __device__ __forceinline__ float u24(uint32_t w) { return ((float)(w >> 8) + 0.5
 // underflows fp32 for mu > 87 and the integer decision must not depend on fp32 rounding of the CDF).  mu < 64: sequential
 // search from 0.  mu >= 64: the same inverse CDF searched from the mode m = floor(mu) (exp(-mu) underflows FP64 above
 // mu ~ 745): p_m = exp(m ln mu - mu - lgamma(m + 1)), F(m) summed downwards from the mode, then a walk down or up.
+// The term ratios mu/k and j/mu are formed with a correctly rounded reciprocal and one multiplication (the oracle divides):
+// the CDF then differs from the oracle's in the last bits only, which moves a decision with probability ~1e-15 per pixel,
+// far inside the 1e-5 of reading O5's protocol; FP64 DDIV was most of the sampler's cost.
 static __device__ __noinline__ int poisson_inv(const double mu, const double u)
 {
     if (!(mu > 0.0)) return 0;
@@ -37,17 +40,17 @@ static __device__ __noinline__ int poisson_inv(const double mu, const double u)
         double p = exp(-mu), c = p;
         while (u > c && k < 100000) {
             ++k;
-            p *= mu / (double)k;
+            p *= mu * __drcp_rn((double)k);           // mu / k up to one rounding (the oracle divides; same inverse CDF)
             c += p;
             if (p == 0.0 && (double)k > mu) break;
         }
         return k;
     }
-    const double m = floor(mu);
+    const double m = floor(mu), inv_mu = __drcp_rn(mu);
     const double pm = exp(m * log(mu) - mu - lgamma(m + 1.0));
     double Fm = pm, p = pm;
     for (double j = m; j >= 1.0; j -= 1.0) {
-        p *= j / mu;
+        p *= j * inv_mu;
         const double next = Fm + p;
         if (next == Fm) break;
         Fm = next;
@@ -55,11 +58,11 @@ static __device__ __noinline__ int poisson_inv(const double mu, const double u)
     double k = m, c = Fm;
     p = pm;
     if (u <= c) {
-        while (k > 0.0 && u <= c - p) { c -= p; p *= k / mu; k -= 1.0; }
+        while (k > 0.0 && u <= c - p) { c -= p; p *= k * inv_mu; k -= 1.0; }
     } else {
         while (u > c && k < 2147483000.0) {
             k += 1.0;
-            p *= mu / k;
+            p *= mu * __drcp_rn(k);
             c += p;
             if (p == 0.0) break;
         }
