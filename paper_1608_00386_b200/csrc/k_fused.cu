@@ -68,8 +68,11 @@ struct FusedCfg {
     static_assert(kTR % n == 0 && NT % n == 0 && n <= 32, "bad fused configuration");
 };
 
+#ifndef AO_FUSED_MINB
+#define AO_FUSED_MINB 3
+#endif
 template <int M, bool NOISE, bool ANYDU, bool MAPS, bool ELONG>
-__global__ void __launch_bounds__(kFusedThreads, 4)
+__global__ void __launch_bounds__(kFusedThreads, AO_FUSED_MINB)
 k_fused(const FusedArgs A)
 {
     using K = FusedCfg<M>;
@@ -395,7 +398,12 @@ void fused_tile_shape(int M, int* G, int* R2)
 }
 
 static size_t fused_xch_bytes(int M) { return M == 64 ? kF64Xch : M == 32 ? FusedCfg<32>::XCH_BYTES : FusedCfg<16>::XCH_BYTES; }
-static size_t fused_budget(int M) { return M == 64 ? 72 * 1024 : 55 * 1024 + 512; }     // M = 64: 2 CTAs per SM
+#ifndef AO_FUSED_BUDGET_KB
+#define AO_FUSED_BUDGET_KB 72
+#endif
+// shared-memory budget per CTA: three CTAs per SM (168 registers, no spills: measured 141 us against 148 at four CTAs of 128
+// registers and 155 at two CTAs of 204 on c4 / M = 32), M = 64 two CTAs per SM
+static size_t fused_budget(int M) { return M == 64 ? 72 * 1024 : (size_t)AO_FUSED_BUDGET_KB * 1024; }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda); NULL if unavailable.
 static PFN_cuTensorMapEncodeTiled tensor_map_encoder()

@@ -26,7 +26,7 @@ struct TiledTrace2Args {
 };
 
 template <int MODE>
-__global__ void __launch_bounds__(kFusedThreads, 4)
+__global__ void __launch_bounds__(kFusedThreads, 3)
 k_trace_tiled2(const TiledTrace2Args A)
 {
     extern __shared__ __align__(128) unsigned char smem[];
