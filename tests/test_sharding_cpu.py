@@ -42,10 +42,21 @@ def _worker(rank, world, port, out):
     psf = torch.zeros(4, 4, dtype=torch.float32)
     for k in range(first, first + count):
         psf += float(k + 1)
+    # every rank loads the C-ABI library itself (one process per GPU); without a CUDA device the library must refuse
+    # loudly instead of falling back to anything (the compute calls are covered on the GPU by tests/test_gpu_*.py)
+    from paper_1608_00386_b200 import binding, inputs
+    lib = binding.load_library()
+    version = lib.ao_version().decode()
+    refused = None
+    if not torch.cuda.is_available():
+        try:
+            binding.Geometry(inputs.make_config(0), device="cuda:0")
+        except Exception as ex:          # RuntimeError from the binding or AoError(AO_ERR_CUDA) from ao_geometry_create
+            refused = type(ex).__name__
     sharding.barrier()
     sharding.sum_over_ranks_(psf)
     t = sharding.max_over_ranks(0.5 + rank)
-    out.put((rank, psf.numpy().copy(), t, first, count))
+    out.put((rank, psf.numpy().copy(), t, first, count, version, refused))
     dist.destroy_process_group()
 
 
@@ -60,7 +71,9 @@ def test_two_rank_gloo_psf_allreduce_and_max_time():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    for rank, psf, t, first, count in res:
+    for rank, psf, t, first, count, version, refused in res:
         assert np.all(psf == float(sum(range(1, 8))))     # 1+...+7 over both ranks
         assert t == 1.5                                    # max over ranks
+        assert "sm_100a" in version and "normal build" in version
+        assert torch.cuda.is_available() or refused in ("RuntimeError", "AoError")
     assert [(r[3], r[4]) for r in res] == [(0, 4), (4, 3)]
