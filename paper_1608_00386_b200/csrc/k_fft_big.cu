@@ -15,7 +15,8 @@
 //   column-interleaved), takes |.|^2 and
 //   - PSF: accumulates the steps of a chunk in registers and adds them to the long exposure once;
 //   - SH: sums the beta x beta detector bins (C = beta: one detector column per CTA).
-// The scratch of a chunk stays L2-resident between the two passes.
+// The scratch of a chunk is sized near the L2 capacity, but ncu --cache-control none shows that most of it is written
+// back to DRAM before the column pass reads it (profiles/r2_big_fft_l2.md): the passes are latency-bound, not DRAM-bound.
 #include <algorithm>
 
 #include "fft_big.cuh"
@@ -252,7 +253,7 @@ size_t psf_scratch_bytes(const ao_geometry* g)
 }
 
 // Steps of the science PSF transformed per launch pair: the column pass sums them in registers, so the
-// long exposure is read and written once per chunk; the scratch of a chunk should stay inside L2.
+// long exposure is read and written once per chunk; the scratch of a chunk is bounded (64 MB).
 int psf_chunk_steps(const ao_geometry* g)
 {
     const size_t per = psf_scratch_bytes(g);
@@ -366,7 +367,7 @@ cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, boo
     }
     if (!sh_big_fast(w)) return launch_sh_big_generic(g, w, phase, api_layout, step_stride, n_steps, scratch, images, st);
     const unsigned batch = (unsigned)(n_sel * nsa);
-    // as many steps per launch pair as the scratch holds (at most 4: the intermediate should stay inside L2)
+    // as many steps per launch pair as the scratch holds (at most 4 and 96 MB: two steps of the NGS sensors measured best)
     const size_t per_step = sh_big_scratch_bytes(g, w);
     int kb = per_step ? (int)std::min<size_t>(4, scratch_bytes / per_step) : 1;
     if (kb < 1) kb = 1;

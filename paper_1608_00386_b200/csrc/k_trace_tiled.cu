@@ -44,19 +44,32 @@ k_trace_tiled2(const TiledTrace2Args A)
     double refsum[2];
     trace2_tile<kFusedThreads, true, MODE>(A.T, sp, S, smem, jfirst, ifirst, A.T.step0 + 2 * kp, acc, refsum);
     const int j0 = jfirst + tid, j1 = j0 + kFusedThreads;
+    const bool in0 = j0 < sp.N, in1 = j1 < sp.N;
+    const int rows_in = min(kTR, sp.N - ifirst);          // CTA-uniform
+    const double scale = sp.scale;
 #pragma unroll
     for (int s = 0; s < kKS; ++s) {
         const int k = 2 * kp + s;
         if (k >= A.n_steps) break;
-        float* out = A.phase + (size_t)k * A.step_stride + A.off[si];
+        float* out = A.phase + (size_t)k * A.step_stride + A.off[si] + (size_t)ifirst * sp.N;
+        if (sp.map == nullptr) {
 #pragma unroll
-        for (int i = 0; i < kTR; ++i) {
-            const int row = ifirst + i;
-            if (row < sp.N) {
-                const float2 f = unpack2(acc[s * kTR + i]);
-                const size_t o0 = (size_t)row * sp.N + j0, o1 = (size_t)row * sp.N + j1;
-                if (j0 < sp.N) out[o0] = (float)(((double)f.x + refsum[0]) * sp.scale + (sp.map ? (double)sp.map[o0] : 0.0));
-                if (j1 < sp.N) out[o1] = (float)(((double)f.y + refsum[1]) * sp.scale + (sp.map ? (double)sp.map[o1] : 0.0));
+            for (int i = 0; i < kTR; ++i) {
+                if (i < rows_in) {
+                    const float2 f = unpack2(acc[s * kTR + i]);
+                    if (in0) out[(size_t)i * sp.N + j0] = (float)(((double)f.x + refsum[0]) * scale);
+                    if (in1) out[(size_t)i * sp.N + j1] = (float)(((double)f.y + refsum[1]) * scale);
+                }
+            }
+        } else {
+            const float* mp = sp.map + (size_t)ifirst * sp.N;
+#pragma unroll
+            for (int i = 0; i < kTR; ++i) {
+                if (i < rows_in) {
+                    const float2 f = unpack2(acc[s * kTR + i]);
+                    if (in0) out[(size_t)i * sp.N + j0] = (float)(((double)f.x + refsum[0]) * scale + (double)__ldg(mp + (size_t)i * sp.N + j0));
+                    if (in1) out[(size_t)i * sp.N + j1] = (float)(((double)f.y + refsum[1]) * scale + (double)__ldg(mp + (size_t)i * sp.N + j1));
+                }
             }
         }
     }
