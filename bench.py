@@ -48,7 +48,7 @@ def ncu_static(steps_per_launch_here: int):
         import csv
         rows = list(csv.reader(open(NCU_RAW_CSV)))
         head = rows[0]
-        data = [r for r in rows[1:] if len(r) == len(head) and r[head.index("Kernel Name")].startswith(("void ao::k_fused", "k_fused", "ao::k_fused"))]
+        data = [r for r in rows[1:] if len(r) == len(head) and "k_fused" in r[head.index("Kernel Name")]]
         units = rows[1] if rows[1][head.index("Kernel Name")] == "" else None
         r = data[0]
 
