@@ -582,3 +582,33 @@ def test_polychromatic_psf_against_the_oracle(n_sub, n_steps):
     from paper_1608_00386_b200 import binding
     with pytest.raises(binding.AoError):
         geo.psf_poly(None, 2, 1, cfg.dt_s)
+
+
+def test_fused64_odd_counts_phase_maps_and_noise():
+    """k_fused64 (M = 64, n = 32: the tile marched twice per subaperture row): odd step counts and odd first steps, a static
+    phase map on two of the six LGS (the kernel reads sp.map), and detector noise through the fused kernel
+    (k_fused64<..., NOISE>) under the protocol of reading O5."""
+    import torch
+    for n_steps, step0 in ((1, 7), (3, 498)):
+        cfg = inputs.make_config(4, n_sub=6, screen_n=1024, n_steps=n_steps, lgs_fft=64, n_layers=7)
+        cfg.sources = cfg.sources[:6]; cfg.wfs = cfg.wfs[:1]; cfg.psf_fft = 0
+        rng = np.random.default_rng(5)
+        cfg.phase_maps = {s: _smooth_map(rng, cfg.grid_n(s), 1.5) for s in (1, 4)}
+        ref = oracle.forward(cfg, step0, n_steps, want_phase=False)
+        geo = _geo(cfg, n_steps)
+        img, slp = geo.sh_images(0, None, step0, n_steps, cfg.dt_s)
+        torch.cuda.synchronize()
+        check_wfs(cfg, geo, ref, 0, img, slp, n_steps, f"k_fused64 {n_steps} steps from {step0}")
+    cfg.noise = inputs.Noise(seed=99, photons_per_subap=4000.0, read_noise_e=2.0)
+    refn = oracle.forward(cfg, 498, 3, want_phase=False, noise_on=True)
+    noisy, slopes = geo.sh_images(0, None, 498, 3, cfg.dt_s, noise=cfg.noise)
+    torch.cuda.synchronize()
+    tot = bad = 0
+    for si, s in enumerate(cfg.sources_of_wfs(0)):
+        for k in range(3):
+            same = np.abs(noisy[k, si].cpu().numpy().astype(np.float64) - refn["noisy"][s][k]) < 0.5
+            tot += same.size; bad += int((~same).sum())
+            ok = same.reshape(same.shape[0], -1).all(axis=1)
+            d = np.abs(slopes[k, si].cpu().numpy().astype(np.float64) - refn["slopes"][s][k])
+            assert d[:, ok].max() <= SLOPE_TOL
+    assert bad <= max(1, int(1e-5 * tot)), (bad, tot)
