@@ -439,16 +439,17 @@ def run_gpu(args):
             return sharding.max_over_ranks(time.perf_counter() - t0, device=dev)
 
         t_e2e = statistics.median([host_call(scr_host) for _ in range(3)])
+        h2d = geo.last_h2d_bytes()                 # what the call uploaded: the part of every screen the K steps read
         t_res = statistics.median([host_call(None) for _ in range(5)])
-        h2d = sum(h.numel() * 4 for h in scr_host)
         d2h = sum(t.numel() * 4 for t in slh) + psfh.numel() * 4
         e2e = {"value": frames_per_step * K * world / t_e2e, "unit": UNIT,
                "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K, "seconds": t_e2e,
                "value_screens_resident": frames_per_step * K * world / t_res, "seconds_screens_resident": t_res,
-               "note": "ao_forward_host, pinned host buffers, host clock around the call (it synchronises), median of 3: H2D of "
-                       "all screens (the run's whole input, once per call, amortised over the K steps), K steps, D2H of all "
-                       "slopes and the long-exposure PSF; value_screens_resident: the same call with the screens already on "
-                       "the device (D2H only, median of 5)"}
+               "h2d_bytes_per_call": h2d, "host_screen_bytes": sum(h.numel() * 4 for h in scr_host),
+               "note": "ao_forward_host, pinned host buffers (all 35 screens of 8192^2 live in host memory), host clock around the "
+                       "call (it synchronises), median of 3: H2D of the part of every screen the K steps read (bounding box of all "
+                       "footprints + margin; counted by the library, ao_last_h2d_bytes), K steps, D2H of all slopes and the "
+                       "long-exposure PSF; value_screens_resident: the same call with the screens already on the device (D2H only, median of 5)"}
         del scr_host
 
     # ---- parity spot check against the oracle + the oracle timed on the host cores (rank 0, N = 1) ----

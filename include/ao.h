@@ -264,9 +264,12 @@ int ao_forward(ao_geometry* g, int64_t step0, int n_steps, double dt_s, const ao
  * synchronises the stream.  slopes_host[w] (nullable per entry) receives WFS w's slopes in the
  * ao_sh_images layout; psf_host (nullable) receives [n_sci][M][M] (sum over the steps).
  * The device staging for the results lives in the workspace (see ao_workspace_bytes).
- * If screens_host is non-NULL, screens_host[l] ([S_l][S_l] floats) is first copied into layer
- * l's borrowed device screen (host->device inside the call): the one call that writes the screens
- * (see ao_layer.screen_dev). */
+ * If screens_host is non-NULL, screens_host[l] ([S_l][S_l] floats, the whole screen) is the host copy of layer l and
+ * the call first uploads, into layer l's borrowed device screen (the one call that writes the screens, see
+ * ao_layer.screen_dev), the part of it that steps [step0, step0 + n_steps) read: the bounding box of all footprints
+ * (periodic wrap included) plus a 24-sample margin; a layer no source sees is not uploaded, a box as large as the screen
+ * uploads all of it.  Device samples outside the box keep their previous contents.  ao_last_h2d_bytes() returns the bytes
+ * the last call uploaded. */
 int ao_forward_host(ao_geometry* g, const float* const* screens_host, int64_t step0, int n_steps,
                     double dt_s, const ao_noise* noise, float* const* slopes_host,
                     float* psf_host, void* cuda_stream);
@@ -277,6 +280,9 @@ int ao_forward_host(ao_geometry* g, const float* const* screens_host, int64_t st
  * rate in TFLOP/s.  packed = 0: scalar FFMA; packed != 0: FFMA2 (fma.rn.f32x2).  Synchronous.
  * Errors: AO_ERR_INVALID_ARG (NULL), AO_ERR_CUDA. */
 int ao_probe_fp32(ao_geometry* g, int packed, double* tflops_out);
+
+/* Bytes of screens uploaded host -> device by the last ao_forward_host call on this handle (0 without screens_host). */
+uint64_t ao_last_h2d_bytes(const ao_geometry* g);
 
 /* Number of kernel launches issued by this handle since creation (all ao_* calls). */
 int64_t ao_launch_count(const ao_geometry* g);

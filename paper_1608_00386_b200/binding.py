@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "AO_OK", 1: "AO_ERR_INVALID_ARG", 2: "AO_ERR_SHAPE", 3: "AO_E
 # every symbol include/ao.h declares
 EXPORTS = ["ao_geometry_create", "ao_geometry_destroy", "ao_workspace_bytes", "ao_set_workspace",
            "ao_phase_elems_per_step", "ao_phase_offset", "ao_wfs_valid", "ao_trace_layers",
-           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_psf_band", "ao_psf_poly", "ao_set_phase_map", "ao_set_sodium", "ao_modes_to_map", "ao_strehl", "ao_strehl_marechal", "ao_forward", "ao_forward_host", "ao_probe_fp32", "ao_launch_count",
+           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_psf_band", "ao_psf_poly", "ao_set_phase_map", "ao_set_sodium", "ao_modes_to_map", "ao_strehl", "ao_strehl_marechal", "ao_forward", "ao_forward_host", "ao_probe_fp32", "ao_last_h2d_bytes", "ao_launch_count",
            "ao_last_error", "ao_version"]
 
 
@@ -92,6 +92,7 @@ def load_library():
     L.ao_forward.argtypes = [vp, i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, i32, vp]
     L.ao_forward_host.argtypes = [vp, C.POINTER(vp), i64, i32, dbl, C.POINTER(ao_noise), C.POINTER(vp), vp, vp]
     L.ao_probe_fp32.argtypes = [vp, i32, C.POINTER(dbl)]
+    L.ao_last_h2d_bytes.argtypes = [vp]; L.ao_last_h2d_bytes.restype = C.c_uint64
     L.ao_launch_count.argtypes = [vp]; L.ao_launch_count.restype = i64
     L.ao_last_error.restype = C.c_char_p
     L.ao_version.restype = C.c_char_p
@@ -244,6 +245,10 @@ class Geometry:
         out = C.c_double(0.0)
         _check(self.lib.ao_probe_fp32(self.handle, int(bool(packed)), C.byref(out)))
         return float(out.value)
+
+    def last_h2d_bytes(self) -> int:
+        """ao_last_h2d_bytes: bytes of screens the last forward_host call uploaded."""
+        return int(self.lib.ao_last_h2d_bytes(self.handle))
 
     def launch_count(self) -> int:
         return int(self.lib.ao_launch_count(self.handle))

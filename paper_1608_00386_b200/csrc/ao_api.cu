@@ -500,6 +500,7 @@ int ao_wfs_valid(const ao_geometry* g, int wfs_index, uint8_t* valid_host)
 }
 
 int64_t ao_launch_count(const ao_geometry* g) { return g ? g->launches : 0; }
+uint64_t ao_last_h2d_bytes(const ao_geometry* g) { return g ? g->h2d_bytes : 0; }
 
 int ao_trace_layers(ao_geometry* g, int64_t step0, int n_steps, double dt_s, float* phase_dev, void* cuda_stream)
 {
@@ -539,6 +540,57 @@ int ao_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, d
     int rc = check_entry(g); if (rc) return rc;
     if (!psf_dev || n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_psf: psf_dev NULL or n_steps < 0");
     return run_psf(g, phase_dev, step0, n_steps, dt_s, psf_dev, accumulate, (cudaStream_t)cuda_stream);
+}
+
+// ao_forward_host: host -> device copy of the part of screen l that steps [step0, step0 + n_steps) read: the bounding box
+// of the footprints of every source that sees the layer, at the first and the last step (the footprint moves linearly
+// in time), plus a margin for the staged boxes of the tiled kernels (they load a few aligned columns and rows beyond the
+// taps); periodic wrap splits the box in up to 2 x 2 pieces.  A box as large as the screen uploads the whole screen.
+static int upload_screen_region(ao_geometry* g, int l, const float* host, int64_t step0, int n_steps, double dt, cudaStream_t st)
+{
+    const LayerP& lp = g->layers[l];
+    const long long S = lp.S;
+    const size_t pitch = sizeof(float) * (size_t)S;
+    auto whole = [&]() {
+        g->h2d_bytes += pitch * (size_t)S;
+        return cudaMemcpyAsync((void*)lp.screen, host, pitch * (size_t)S, cudaMemcpyHostToDevice, st);
+    };
+    if (n_steps <= 0) return AO_OK;
+    bool any = false;
+    double umin = 0, umax = 0, vmin = 0, vmax = 0;
+    for (const SourceP& sp : g->sources) {
+        if (!(lp.height < sp.H)) continue;
+        const double gamma = 1.0 - lp.height * sp.inv_H, x0 = -0.5 * (double)(sp.N - 1) * sp.d, c = 0.5 * (double)(S - 1);
+        const double du = gamma * sp.d * lp.inv_pitch;
+        for (int e = 0; e < 2; ++e) {
+            const double t = (double)(step0 + (e ? n_steps - 1 : 0)) * dt;
+            const double u0 = (gamma * x0 + lp.height * sp.thx - lp.wx * t) * lp.inv_pitch + c, u1 = u0 + (sp.N - 1) * du;
+            const double v0 = (gamma * x0 + lp.height * sp.thy - lp.wy * t) * lp.inv_pitch + c, v1 = v0 + (sp.N - 1) * du;
+            if (!any) { umin = std::min(u0, u1); umax = std::max(u0, u1); vmin = std::min(v0, v1); vmax = std::max(v0, v1); any = true; }
+            umin = std::min(umin, std::min(u0, u1)); umax = std::max(umax, std::max(u0, u1));
+            vmin = std::min(vmin, std::min(v0, v1)); vmax = std::max(vmax, std::max(v0, v1));
+        }
+    }
+    if (!any) return AO_OK;                                   // no source sees this layer: nothing is read
+    const long long margin = 24;
+    const long long c_lo = (long long)floor(umin) - margin, c_hi = (long long)floor(umax) + 1 + margin;
+    const long long r_lo = (long long)floor(vmin) - margin, r_hi = (long long)floor(vmax) + 1 + margin;
+    const long long W = c_hi - c_lo + 1, H = r_hi - r_lo + 1;
+    if (W >= S || H >= S || fabs(umin) > 1e15 || fabs(vmin) > 1e15) { AO_CUDA(whole(), "screen upload"); return AO_OK; }
+    const long long cw = ((c_lo % S) + S) % S, rw = ((r_lo % S) + S) % S;
+    const long long cpart[2][2] = {{cw, std::min(W, S - cw)}, {0, W - std::min(W, S - cw)}};      // {start, count}
+    const long long rpart[2][2] = {{rw, std::min(H, S - rw)}, {0, H - std::min(H, S - rw)}};
+    float* dev = const_cast<float*>(lp.screen);
+    for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) {
+            const long long r0 = rpart[a][0], nr = rpart[a][1], c0 = cpart[b][0], nc = cpart[b][1];
+            if (nr <= 0 || nc <= 0) continue;
+            const size_t off = (size_t)r0 * S + (size_t)c0;
+            AO_CUDA(cudaMemcpy2DAsync(dev + off, pitch, host + off, pitch, sizeof(float) * (size_t)nc, (size_t)nr,
+                                      cudaMemcpyHostToDevice, st), "screen region upload");
+            g->h2d_bytes += sizeof(float) * (size_t)nc * (size_t)nr;
+        }
+    return AO_OK;
 }
 
 // Shared by ao_forward and ao_forward_host: all WFS (slopes only) and the PSF for steps [step0, step0 + n_steps).
@@ -762,11 +814,12 @@ int ao_forward_host(ao_geometry* g, const float* const* screens_host, int64_t st
     if (n_steps < 0) return fail(AO_ERR_INVALID_ARG, "ao_forward_host: n_steps < 0");
     if (!g->ws || g->ws_chunk < 1) return fail(AO_ERR_WORKSPACE, "ao_forward_host needs a workspace");
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    g->h2d_bytes = 0;
     if (screens_host)
         for (size_t l = 0; l < g->layers.size(); ++l) {
             if (!screens_host[l]) return fail(AO_ERR_INVALID_ARG, "ao_forward_host: screens_host[l] is NULL");
-            AO_CUDA(cudaMemcpyAsync((void*)g->layers[l].screen, screens_host[l],
-                                    sizeof(float) * (size_t)g->layers[l].S * g->layers[l].S, cudaMemcpyHostToDevice, st), "screen upload");
+            rc = upload_screen_region(g, (int)l, screens_host[l], step0, n_steps, dt_s, st);
+            if (rc) return rc;
         }
     const WsView v = ws_view(g);
     const bool want_psf = psf_host && g->psf_fft && !g->sci.src.empty();

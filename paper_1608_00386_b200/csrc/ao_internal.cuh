@@ -117,6 +117,7 @@ struct ao_geometry {
     size_t ws_bytes = 0;
     int ws_chunk = 0;                 // steps per internal chunk that fit the workspace
     int64_t launches = 0;
+    uint64_t h2d_bytes = 0;           // bytes of screens uploaded by the last ao_forward_host
     int sm_count = 148;
     int device = 0;                   // the CUDA device the handle was created on (made current by every call)
     // ao_forward: high-priority side stream for the workspace users (big-FFT sensors, PSF), fork / join events

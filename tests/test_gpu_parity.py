@@ -264,14 +264,28 @@ def test_forward_host_matches_device_path():
     psf = torch.empty((len(cfg.science_sources()), cfg.psf_fft, cfg.psf_fft), dtype=torch.float32).pin_memory()
     scr = [torch.from_numpy(l.screen).pin_memory() for l in cfg.layers]
     for s in geo.screens:
-        s.zero_()                                          # the call must upload the screens itself
+        s.fill_(float("nan"))                              # the call must upload what it reads itself: anything it misses is NaN
     geo.forward_host(0, 3, cfg.dt_s, sl, psf, screens_host=scr)
+    full = sum(l.n * l.n * 4 for l in cfg.layers)
+    assert 0 < geo.last_h2d_bytes() < full                 # only the footprints' bounding box of every screen travels
+    assert all(bool(torch.isfinite(t).all()) for t in sl) and bool(torch.isfinite(psf).all())
     for w in range(len(cfg.wfs)):
         for si, s in enumerate(cfg.sources_of_wfs(w)):
             for k in range(3):
                 assert np.abs(sl[w][k, si].numpy() - ref["slopes"][s][k]).max() <= SLOPE_TOL
     for di, s in enumerate(cfg.science_sources()):
         assert rel_l2(psf[di].numpy(), ref["psf"][s]) <= IMAGE_TOL
+    # far into the run the footprints have drifted across the periodic screen edge: the box is uploaded in pieces
+    for s in geo.screens:
+        s.fill_(float("nan"))
+    ref2 = oracle.forward(cfg, 4000, 2, want_phase=False)
+    geo.forward_host(4000, 2, cfg.dt_s, [t[:2] for t in sl], psf, screens_host=scr)
+    for w in range(len(cfg.wfs)):
+        for si, s in enumerate(cfg.sources_of_wfs(w)):
+            for k in range(2):
+                assert np.abs(sl[w][k, si].numpy() - ref2["slopes"][s][k]).max() <= SLOPE_TOL
+    for di, s in enumerate(cfg.science_sources()):
+        assert rel_l2(psf[di].numpy(), ref2["psf"][s]) <= IMAGE_TOL
 
 
 @pytest.mark.parametrize("n_sub,psf_fft,n_steps", [(4, 64, 2), (20, None, 10), (40, None, 2), (20, 4096, 1), (80, None, 1)])
