@@ -73,6 +73,12 @@ struct __align__(16) LayerT {
     double vrel[kKS];     // row coordinate of tile row 0 relative to box row 0
     u64 uf[kKS];          // (column coordinate of tile column 0 - box column 0) 2^32
 };
+// Unit march (du = 1): vrel / uf are replaced, in place, by what its consumers need: the box row of the top tap of tile
+// row 0 and the box column of tile column 0 (per step), and the two fractional weights of the whole tile.
+struct UnitT { float fy[kKS], fx[kKS]; int row[kKS], col[kKS]; };
+static_assert(sizeof(UnitT) == sizeof(double) * kKS + sizeof(u64) * kKS, "UnitT overlays LayerT::vrel and LayerT::uf");
+__device__ __forceinline__ UnitT* unit_of(LayerT& T) { return reinterpret_cast<UnitT*>(&T.vrel[0]); }
+__device__ __forceinline__ const UnitT* unit_of(const LayerT& T) { return reinterpret_cast<const UnitT*>(&T.vrel[0]); }
 
 struct __align__(16) Trace2Shared {
     uint64_t full_bar[kT2MaxStages], empty_bar[kT2MaxStages];
@@ -262,10 +268,21 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         T.du = du; T.du_hi = (int)floor(du);
         const unsigned long long f = __double2ull_rn((du - (double)T.du_hi) * 4294967296.0);
         T.duf = f > 0xffffffffull ? 0xffffffffu : (unsigned)f;
+        if (MODE == 3) {                                           // du = 1: one cell offset and one weight pair per step
+            UnitT u;
 #pragma unroll
-        for (int s = 0; s < kKS; ++s) {
-            T.uf[s] = __double2ull_rn((uf[s] - (double)cmin) * 4294967296.0);
-            T.vrel[s] = vf[s] - (double)rmin;
+            for (int s = 0; s < kKS; ++s) {
+                const double ur = uf[s] - (double)cmin, vr = vf[s] - (double)rmin, fu = floor(ur), fv = floor(vr);
+                u.col[s] = (int)fu; u.fx[s] = (float)(ur - fu);
+                u.row[s] = (int)fv; u.fy[s] = (float)(vr - fv);
+            }
+            *unit_of(T) = u;
+        } else {
+#pragma unroll
+            for (int s = 0; s < kKS; ++s) {
+                T.uf[s] = __double2ull_rn((uf[s] - (double)cmin) * 4294967296.0);
+                T.vrel[s] = vf[s] - (double)rmin;
+            }
         }
     }
     __syncthreads();
@@ -356,6 +373,21 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             issue(l + ns, l - m * ns);
         }
         const LayerT& T = L[a];
+        if (MODE == 3) {
+            // du = 1: every per-thread quantity is the layer's (row, column, fx, fy) plus the thread's column index
+            const uint32_t tile_u = tiles_s + (uint32_t)stage * tile_bytes;
+            if (!AO_DBG_ON(A, 2)) mbar_wait(&S.full_bar[stage], par);
+            const UnitT u = *unit_of(T);
+            const uint32_t b0 = tile_u + ((uint32_t)u.row[0] * kUnitPitch + (uint32_t)u.col[0]) * 4u;
+            const uint32_t b1 = tile_u + ((uint32_t)u.row[1] * kUnitPitch + (uint32_t)u.col[1]) * 4u;
+            const float r0f = lds_f32(b0 + (uint32_t)(tid & ~31) * 4u), r1f = lds_f32(b0 + (uint32_t)((tid & ~31) + NT) * 4u);
+            const u64 ref = pack2(r0f, r1f);
+            if (REFSUM) { refsum[0] += (double)r0f; refsum[1] += (double)r1f; }
+            if (!AO_DBG_ON(A, 1)) {
+                t2_march_unit<0>(acc, b0 + (uint32_t)tid * 4u, b0 + (uint32_t)(tid + NT) * 4u, pack2(u.fx[0], u.fx[0]), ref, 1.0f - u.fy[0], u.fy[0]);
+                t2_march_unit<kTR>(acc, b1 + (uint32_t)tid * 4u, b1 + (uint32_t)(tid + NT) * 4u, pack2(u.fx[1], u.fx[1]), ref, 1.0f - u.fy[1], u.fy[1]);
+            }
+        } else {
         const uint32_t pb = (uint32_t)T.pitch * 4u;
         const u64 du64 = ((u64)(unsigned)T.du_hi << 32) | (u64)T.duf;
         const u64 uf0 = T.uf[0], uf1 = T.uf[1];
@@ -363,12 +395,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         const u64 colA = (u64)(unsigned)tid * du64, colB = colA + (u64)NT * du64;
         const u64 colW = (u64)(unsigned)(tid & ~31) * du64;
         if (!AO_DBG_ON(A, 2)) mbar_wait(&S.full_bar[stage], par);
-        int ro0, ro1;
-        float fy0 = 0.0f, fy1 = 0.0f;
-        if (MODE == 3) {                       // du = 1: top row and weight of the whole tile from the FP64 origin
-            const double v0 = T.vrel[0], v1 = T.vrel[1], f0 = floor(v0), f1 = floor(v1);
-            ro0 = (int)f0; ro1 = (int)f1; fy0 = (float)(v0 - f0); fy1 = (float)(v1 - f1);
-        } else { ro0 = R0[stage * kKS]; ro1 = R0[stage * kKS + 1]; }
+        const int ro0 = R0[stage * kKS], ro1 = R0[stage * kKS + 1];
         u64 ref;
         {
             const u64 a0 = uf0 + colW, a1 = a0 + (u64)NT * du64;
@@ -385,8 +412,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
                 const uint32_t rowb = tile_s + (uint32_t)ro0 * pb;
                 const uint32_t t0 = rowb + (uint32_t)(U0 >> 32) * 4u, t1 = rowb + (uint32_t)(U1 >> 32) * 4u;
                 const uint32_t wt_s = w_s + (uint32_t)(stage * kKS + 0) * (kTR * 16);
-                if (MODE == 3) t2_march_unit<0>(acc, t0, t1, fx, ref, 1.0f - fy0, fy0);
-                else if (MODE == 2) t2_march_quad<0>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 0) * 4));
+                if (MODE == 2) t2_march_quad<0>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 0) * 4));
                 else if (MODE == 1) t2_march_any<0>(acc, t0, t1, pb, fx, ref, wt_s);
                 else t2_march<0>(acc, t0, t1, fx, ref, wt_s);
             }
@@ -396,11 +422,11 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
                 const uint32_t rowb = tile_s + (uint32_t)ro1 * pb;
                 const uint32_t t0 = rowb + (uint32_t)(U0 >> 32) * 4u, t1 = rowb + (uint32_t)(U1 >> 32) * 4u;
                 const uint32_t wt_s = w_s + (uint32_t)(stage * kKS + 1) * (kTR * 16);
-                if (MODE == 3) t2_march_unit<kTR>(acc, t0, t1, fx, ref, 1.0f - fy1, fy1);
-                else if (MODE == 2) t2_march_quad<kTR>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 1) * 4));
+                if (MODE == 2) t2_march_quad<kTR>(acc, t0, t1, pb, fx, ref, wt_s, smem_u32(G + (stage * kKS + 1) * 4));
                 else if (MODE == 1) t2_march_any<kTR>(acc, t0, t1, pb, fx, ref, wt_s);
                 else t2_march<kTR>(acc, t0, t1, fx, ref, wt_s);
             }
+        }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&S.empty_bar[stage]);
