@@ -249,11 +249,10 @@ int ao_strehl_marechal(ao_geometry* g, const float* phase_dev, int n_steps, floa
 
 /* ao_forward -- the whole step with DEVICE buffers: ray-trace + every WFS (slopes only, noiseless unless
  * `noise`) + every science PSF for n_steps steps (the per-time-step forward model).
- * Same results as one ao_sh_images(phase_dev = NULL, images_dev = NULL) per WFS plus ao_psf(phase_dev = NULL),
- * but the workspace users (big-FFT sensors, PSF) run on a library-owned high-priority side stream concurrently
- * with the sensors that need no workspace (the fused ray-trace + SH + CoG kernel) on `cuda_stream`; the side
- * stream is forked from and joined back into `cuda_stream` by events, so the call is asynchronous on `cuda_stream` like
- * every other call.  slopes_dev[w] (nullable per entry): ao_sh_images slopes layout of WFS w.
+ * Same results as one ao_sh_images(phase_dev = NULL, images_dev = NULL) per WFS plus ao_psf(phase_dev = NULL) (ao_psf_poly
+ * while a band is set), submitted in order on `cuda_stream`: the workspace users (big-FFT sensors, PSF) first, then the
+ * sensors that need no workspace (the fused ray-trace + SH + CoG kernels).  Asynchronous like every other call.
+ * slopes_dev[w] (nullable per entry): ao_sh_images slopes layout of WFS w.
  * psf_dev (nullable): [n_sci][M][M], += if accumulate else =.  Needs a workspace if any big WFS or PSF runs. */
 int ao_forward(ao_geometry* g, int64_t step0, int n_steps, double dt_s, const ao_noise* noise,
                float* const* slopes_dev, float* psf_dev, int accumulate, void* cuda_stream);

@@ -80,9 +80,6 @@ static void destroy(ao_geometry* g)
     cudaFree(g->d_pupil_amp); cudaFree(g->d_layers); cudaFree(g->d_sources);
     cudaFree(g->d_psf_tw); cudaFree(g->d_psf_pre);
     free_band(g);
-    if (g->ev_fork) cudaEventDestroy(g->ev_fork);
-    if (g->ev_join) cudaEventDestroy(g->ev_join);
-    if (g->side) cudaStreamDestroy(g->side);
     for (auto& w : g->wfs) {
         cudaFree(w.d_amp); cudaFree(w.d_valid); cudaFree(w.d_w2m); cudaFree(w.d_tw); cudaFree(w.d_twf); cudaFree(w.d_pre); cudaFree(w.fused_items);
         free_sodium(w);
@@ -118,7 +115,9 @@ static Plan make_plan(const ao_geometry* g)
         p.slopes += align256(sizeof(float) * n_sel * 2 * nsa);
         if (w.big) {
             size_t s = sh_big_scratch_bytes(g, w);
-            if (2 * s <= ((size_t)96 << 20)) s *= 2;         // two steps per launch pair up to 96 MB of intermediate (measured: 119 us per step against 126 with one)
+            int kb = 8;                                      // up to 8 steps per launch pair within 768 MB of intermediate
+            while (kb > 1 && (size_t)kb * s > ((size_t)768 << 20)) --kb;
+            s *= (size_t)kb;
             if (s > p.scratch) p.scratch = s;
             const size_t im = align256(sizeof(float) * n_sel * nsa * w.P * w.P);
             if (im > p.bigimg) p.bigimg = im;
@@ -315,15 +314,6 @@ int ao_geometry_create(const ao_pupil* pupil, const ao_wfs* wfs, int n_wfs, cons
     cudaGetDevice(&dev);
     g->device = dev;
     cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    int prio_least = 0, prio_greatest = 0;
-    cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest);
-    if (cudaStreamCreateWithPriority(&g->side, cudaStreamNonBlocking, prio_greatest) != cudaSuccess ||
-        cudaEventCreateWithFlags(&g->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&g->ev_join, cudaEventDisableTiming) != cudaSuccess) {
-        g->side = nullptr; g->ev_fork = nullptr; g->ev_join = nullptr;      // ao_forward then runs on one stream
-        cudaGetLastError();
-    }
-
     g->Np = pupil->n; g->pitch = pupil->pitch_m; g->lambda_ref = lambda_ref_m;
     const size_t np2 = (size_t)g->Np * g->Np;
     for (size_t i = 0; i < np2; ++i) { g->sumA2 += (double)pupil->amp_host[i] * pupil->amp_host[i]; g->sumA += (double)pupil->amp_host[i]; }
@@ -593,48 +583,25 @@ static int upload_screen_region(ao_geometry* g, int l, const float* host, int64_
     return AO_OK;
 }
 
-// Shared by ao_forward and ao_forward_host: all WFS (slopes only) and the PSF for steps [step0, step0 + n_steps).
-// The workspace users (big-FFT sensors, PSF: many short, latency-bound launches) run in order on the library's
-// HIGH-priority side stream, forked from and joined into `st`; the workspace-free fused sensors (one long launch
-// that fills every SM) run on `st`.  With the priorities this way round the block scheduler hands freed SM slots
-// to the short kernels first, so both chains progress together instead of one behind the other.
+// Shared by ao_forward and ao_forward_host: all WFS (slopes only) and the PSF for steps [step0, step0 + n_steps), in order
+// on the caller's stream: the workspace users first (big-FFT sensors, PSF: many short launches), then the fused sensors.
+// A library-owned high-priority side stream for the workspace users was measured and removed: the fused kernel's CTAs hold the
+// whole register file of an SM, nothing overlaps, and the fork / join cost 4 us per step on c4 and 50 us per step on c3.
 static int forward_chunk(ao_geometry* g, int64_t step0, int n_steps, double dt_s, const ao_noise* noise,
                          float* const* slopes, float* psf, int accumulate, cudaStream_t st)
 {
-    int rc;
+    int rc = AO_OK;
     const bool want_psf = psf && g->psf_fft && !g->sci.src.empty();
-    bool any_ws = want_psf, any_free = false;
-    std::vector<char> on_side(g->wfs.size(), 0);
-    for (size_t wi = 0; wi < g->wfs.size(); ++wi) {
-        const WfsH& w = g->wfs[wi];
-        if (!slopes || !slopes[wi] || w.grp.src.empty()) continue;
-        const bool ws_free = (!w.big || w.M == 64) && fused_supported(g, w, dt_s);
-        on_side[wi] = ws_free ? 0 : 1;
-        (ws_free ? any_free : any_ws) = true;
-    }
-    const bool fork = g->side && any_ws && any_free;
-    cudaStream_t sw = fork ? g->side : st;                  // stream of the workspace users
-    if (fork) {
-        AO_CUDA(cudaEventRecord(g->ev_fork, st), "fork record");
-        AO_CUDA(cudaStreamWaitEvent(g->side, g->ev_fork, 0), "fork wait");
-    }
-    // the short kernels are submitted first so that they start at once; the long fused launch fills in behind them
-    rc = AO_OK;
     for (int pass = 0; pass < 2 && rc == AO_OK; ++pass) {
         for (size_t wi = 0; wi < g->wfs.size() && rc == AO_OK; ++wi) {
             const WfsH& w = g->wfs[wi];
-            if (!slopes || !slopes[wi] || w.grp.src.empty() || (on_side[wi] != 0) != (pass == 0)) continue;
-            rc = run_wfs(g, (int)wi, nullptr, step0, n_steps, dt_s, noise, nullptr, slopes[wi], on_side[wi] ? sw : st);
+            if (!slopes || !slopes[wi] || w.grp.src.empty()) continue;
+            const bool fused = (!w.big || w.M == 64) && fused_supported(g, w, dt_s);
+            if (fused != (pass == 1)) continue;
+            rc = run_wfs(g, (int)wi, nullptr, step0, n_steps, dt_s, noise, nullptr, slopes[wi], st);
         }
         if (pass == 0 && want_psf && rc == AO_OK)
-            rc = run_psf(g, nullptr, step0, n_steps, dt_s, psf, accumulate, sw, g->band.n > 0);
-    }
-    // the side stream is joined on every path, also after a failed launch: work already queued there must stay
-    // ordered before whatever the caller submits next on `st`
-    if (fork) {
-        const cudaError_t e1 = cudaEventRecord(g->ev_join, g->side);
-        const cudaError_t e2 = e1 == cudaSuccess ? cudaStreamWaitEvent(st, g->ev_join, 0) : e1;
-        if (e2 != cudaSuccess && rc == AO_OK) return cuda_fail(e2, "join");
+            rc = run_psf(g, nullptr, step0, n_steps, dt_s, psf, accumulate, st, g->band.n > 0);
     }
     return rc;
 }

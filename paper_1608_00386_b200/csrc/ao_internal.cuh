@@ -120,9 +120,6 @@ struct ao_geometry {
     uint64_t h2d_bytes = 0;           // bytes of screens uploaded by the last ao_forward_host
     int sm_count = 148;
     int device = 0;                   // the CUDA device the handle was created on (made current by every call)
-    // ao_forward: high-priority side stream for the workspace users (big-FFT sensors, PSF), fork / join events
-    cudaStream_t side = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
 namespace ao {

@@ -258,10 +258,10 @@ int psf_chunk_steps(const ao_geometry* g)
 {
     const size_t per = psf_scratch_bytes(g);
     if (per == 0) return 1;
-    const size_t budget = (size_t)64 << 20;
+    const size_t budget = (size_t)3 << 29;                   // 1.5 GB of scratch at most
     size_t ks = budget / per;
     if (ks < 1) ks = 1;
-    if (ks > 8) ks = 8;
+    if (ks > 16) ks = 16;
     return (int)ks;
 }
 
@@ -369,9 +369,8 @@ cudaError_t launch_sh_big(ao_geometry* g, const WfsH& w, const float* phase, boo
     const unsigned batch = (unsigned)(n_sel * nsa);
     // as many steps per launch pair as the scratch holds (at most 4 and 96 MB: two steps of the NGS sensors measured best)
     const size_t per_step = sh_big_scratch_bytes(g, w);
-    int kb = per_step ? (int)std::min<size_t>(4, scratch_bytes / per_step) : 1;
+    int kb = per_step ? (int)std::min<size_t>(8, scratch_bytes / per_step) : 1;
     if (kb < 1) kb = 1;
-    while (kb > 1 && (size_t)kb * per_step > ((size_t)96 << 20)) --kb;
     while (kb > 1 && (size_t)kb * batch > 65535u) --kb;    // the batch is gridDim.y (ao_geometry_create bounds one step)
     for (int k = 0; k < n_steps; k += kb) {
         const int kn = n_steps - k < kb ? n_steps - k : kb;

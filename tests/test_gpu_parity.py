@@ -351,7 +351,7 @@ def test_low_altitude_source_takes_the_two_row_march():
 
 
 def test_forward_matches_separate_calls():
-    """ao_forward (fused sensors on the library's side stream, big-FFT sensors and PSF on the caller's) gives
+    """ao_forward (big-FFT sensors and PSF first, then the fused sensors, all on the caller's stream) gives
     the same slopes and long-exposure PSF as ao_sh_images per WFS plus ao_psf, bit for bit."""
     import torch
     cfg = inputs.make_config(3, n_sub=8, screen_n=512, n_steps=3)
