@@ -54,15 +54,25 @@ k_big_rows(const BigRowArgs A)
     const float* am = A.amp + rowoff;
     const float2 pa = row_on ? A.pre[a] : make_float2(0.0f, 0.0f);
     float2* out = A.T + ((size_t)b * n + (row_on ? a : 0)) * M;
+    // all global loads of the thread's 16 input points are issued before the first use (predicated, no branch): the row
+    // pass used to wait for each load in turn (30 % of its stall samples)
+    float ph_r[16], am_r[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const int i = tb + k * (M / 16);
+        const bool on = row_on && i < n;
+        ph_r[k] = on ? __ldg(ph + i) : 0.0f;
+        am_r[k] = on ? __ldg(am + i) : 0.0f;
+    }
     big_fft<LOGM>(tb, sm, 1, r * K::PADM, A.tw,
         [&](int i) {
+            const int k = (i - tb) >> (LOGM - 4);                  // first pass: point i = tb + k M/16 (folds to a constant)
             float2 v = make_float2(0.0f, 0.0f);
             if (row_on && i < n) {
-                const float Am = __ldg(am + i);
                 float s, c;
-                sincos_reduced(__ldg(ph + i), &s, &c);
+                sincos_reduced(ph_r[k], &s, &c);
                 const float2 w = cmulf(pa, __ldg(A.pre + i));
-                v = cmulf(make_float2(Am * c, Am * s), w);
+                v = cmulf(make_float2(am_r[k] * c, am_r[k] * s), w);
             }
             return v;
         },
