@@ -93,7 +93,7 @@ k_fused(const FusedArgs A)
     // ---- phase A: ray-trace of the 16 x 256 tile, two steps, into registers ----
     u64 acc[kKS * kTR];
     double refsum[2];                                      // unused: |FFT|^2 is piston-invariant per subaperture
-    trace2_tile<NT, false, ANYDU ? 1 : 0>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, refsum);
+    trace2_tile<NT, false, ANYDU ? 1 : 0, true>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, refsum, it.cnt * n);
     __syncthreads();                                       // stages are dead: shared memory becomes the exchange buffer
 
     // ---- phase B: image formation, one (subaperture row, column slot) round at a time ----

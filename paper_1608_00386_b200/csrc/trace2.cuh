@@ -201,13 +201,17 @@ __device__ __forceinline__ void t2_march_unit(u64 (&acc)[kKS * kTR], const uint3
 // `dyn`: dynamic shared memory, 128-byte aligned: [ns][rows][pitch] floats, then trace2_sched_bytes(n_layers).
 // All NT threads call it.  On return every thread has finished reading the stages, but other warps may not
 // have: __syncthreads() before reusing the memory.
-template <int NT, bool REFSUM, int MODE>
+// PARTIAL: only the first ncols_used columns of the tile are wanted (a work item with fewer subapertures than the
+// tile holds): a warp whose 32 columns tid and whose columns tid + NT all lie beyond them skips the row marches (its
+// acc stays zero); it still takes its producer turns and barrier arrivals.
+template <int NT, bool REFSUM, int MODE, bool PARTIAL = false>
 __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& sp, Trace2Shared& S, unsigned char* dyn,
                                             const int jfirst, const int ifirst, const long long step_first,
-                                            u64 (&acc)[kKS * kTR], double (&refsum)[2])
+                                            u64 (&acc)[kKS * kTR], double (&refsum)[2], const int ncols_used = 2 * NT)
 {
     constexpr int NCOL = 2 * NT;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool idle = PARTIAL && (int)(tid & ~31u) >= ncols_used;
     const int pitch = A.pitch, ns = A.ns;
     const int tile_floats = A.rows * pitch;
     float* tiles = reinterpret_cast<float*>(dyn);
@@ -383,7 +387,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             const float r0f = lds_f32(b0 + (uint32_t)(tid & ~31) * 4u), r1f = lds_f32(b0 + (uint32_t)((tid & ~31) + NT) * 4u);
             const u64 ref = pack2(r0f, r1f);
             if (REFSUM) { refsum[0] += (double)r0f; refsum[1] += (double)r1f; }
-            if (!AO_DBG_ON(A, 1)) {
+            if (!AO_DBG_ON(A, 1) && !idle) {
                 t2_march_unit<0>(acc, b0 + (uint32_t)tid * 4u, b0 + (uint32_t)(tid + NT) * 4u, pack2(u.fx[0], u.fx[0]), ref, 1.0f - u.fy[0], u.fy[0]);
                 t2_march_unit<kTR>(acc, b1 + (uint32_t)tid * 4u, b1 + (uint32_t)(tid + NT) * 4u, pack2(u.fx[1], u.fx[1]), ref, 1.0f - u.fy[1], u.fy[1]);
             }
@@ -405,7 +409,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             if (REFSUM) { refsum[0] += (double)r0f; refsum[1] += (double)r1f; }
         }
         const float k32 = 2.3283064365386963e-10f;             // 2^-32
-        if (!AO_DBG_ON(A, 1)) {
+        if (!AO_DBG_ON(A, 1) && !idle) {
             {
                 const u64 U0 = uf0 + colA, U1 = uf0 + colB;
                 const u64 fx = pack2(__uint2float_rn((unsigned)U0) * k32, __uint2float_rn((unsigned)U1) * k32);
