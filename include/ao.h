@@ -177,6 +177,26 @@ int ao_centroids(ao_geometry* g, int wfs_index, const float* images_dev, int n_i
 int ao_psf(ao_geometry* g, const float* phase_dev, int64_t step0, int n_steps, double dt_s,
            float* psf_dev, int accumulate, void* cuda_stream);
 
+/* ao_psf_static -- ao_psf for ONE science direction from a phase buffer, for callers that may not allocate (CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc) and so cannot lend a workspace either.  Same
+ * operation and kernels as ao_psf (section 2.8; reading O7):
+ *   psf_dev = (accumulate ? psf_dev : 0) + sum_{k < n_steps} |DFT_M(A exp(i phi_k))|^2 / (M^2 sum A^2)
+ * for science direction `direction` (index among the science directions, ascending source order).
+ *   phase_dev : DEVICE, ao_trace_layers layout, n_steps steps (required: this call does no ray-trace).
+ *   psf_dev   : DEVICE, [M][M] floats of that one direction, caller-owned.
+ * The intermediate of the two-pass FFT (pupil n x M complex floats) lives in a static device array of
+ * AO_PSF_STATIC_MAX_BYTES that every GPU loading the library holds until the process exits; the call makes no
+ * cudaMalloc / cudaFree and calls no allocating library routine, needs no workspace, and is asynchronous on `cuda_stream`.
+ * pupil n * M * 8 > AO_PSF_STATIC_MAX_BYTES is rejected with AO_ERR_UNSUPPORTED (c3 / c4: 960 x 2048 x 8 = 15.7 MB fits).
+ * All calls on one device share the array (whatever the handle): it keeps the previous call's intermediate, which the
+ * row pass overwrites in full before it is read, so nothing is cleared; two calls that overlap on the GPU (different
+ * streams, or two host threads) RACE on it and give wrong PSFs -- serialise them on one stream or with events.
+ * Errors: AO_ERR_INVALID_ARG (NULL, direction out of range, n_steps < 0, no science direction),
+ *   AO_ERR_UNSUPPORTED (size beyond the static scratch), AO_ERR_CUDA. */
+#define AO_PSF_STATIC_MAX_BYTES (16u << 20)
+int ao_psf_static(ao_geometry* g, int direction, const float* phase_dev, int n_steps, float* psf_dev,
+                  int accumulate, void* cuda_stream);
+
 /* ao_set_psf_band / ao_psf_poly -- polychromatic science PSF (section 2.8: "The user select the wavelength at
  * which the PSF is computed and the pixelscale ... The user may desire more wavelengths, considering a bandwidth"; DESIGN.md
  * section 3 reading O8).  The detector pixels keep the angular size lambda_s / (M d_p) of the science directions' own

@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "AO_OK", 1: "AO_ERR_INVALID_ARG", 2: "AO_ERR_SHAPE", 3: "AO_E
 # every symbol include/ao.h declares
 EXPORTS = ["ao_geometry_create", "ao_geometry_destroy", "ao_workspace_bytes", "ao_set_workspace",
            "ao_phase_elems_per_step", "ao_phase_offset", "ao_wfs_valid", "ao_trace_layers",
-           "ao_sh_images", "ao_centroids", "ao_psf", "ao_set_psf_band", "ao_psf_poly", "ao_set_phase_map", "ao_set_sodium", "ao_modes_to_map", "ao_strehl", "ao_strehl_marechal", "ao_forward", "ao_forward_host", "ao_probe_fp32", "ao_last_h2d_bytes", "ao_launch_count",
+           "ao_sh_images", "ao_centroids", "ao_psf", "ao_psf_static", "ao_set_psf_band", "ao_psf_poly", "ao_set_phase_map", "ao_set_sodium", "ao_modes_to_map", "ao_strehl", "ao_strehl_marechal", "ao_forward", "ao_forward_host", "ao_probe_fp32", "ao_last_h2d_bytes", "ao_launch_count",
            "ao_last_error", "ao_version"]
 
 
@@ -82,6 +82,7 @@ def load_library():
     L.ao_sh_images.argtypes = [vp, i32, vp, i64, i32, dbl, C.POINTER(ao_noise), vp, vp, vp]
     L.ao_centroids.argtypes = [vp, i32, vp, i32, vp, vp]
     L.ao_psf.argtypes = [vp, vp, i64, i32, dbl, vp, i32, vp]
+    L.ao_psf_static.argtypes = [vp, i32, vp, i32, vp, i32, vp]
     L.ao_set_psf_band.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), i32]
     L.ao_psf_poly.argtypes = [vp, vp, i64, i32, dbl, vp, i32, vp]
     L.ao_set_phase_map.argtypes = [vp, i32, vp]
@@ -299,6 +300,12 @@ class Geometry:
         if psf is None:
             psf = torch.zeros((n_sci, M, M), dtype=torch.float32, device=self.device)
         _check(self.lib.ao_psf(self.handle, _ptr(phase), step0, n_steps, dt_s, _ptr(psf), int(accumulate), _stream()))
+        return psf
+
+    def psf_static(self, direction: int, phase, n_steps: int, psf, accumulate=False):
+        """ao_psf_static: PSF of one science direction with the FFT intermediate in the library's static device array
+        (no workspace, no allocation).  `psf` [M][M] is caller-owned: this binding allocates nothing either."""
+        _check(self.lib.ao_psf_static(self.handle, int(direction), _ptr(phase), int(n_steps), _ptr(psf), int(accumulate), _stream()))
         return psf
 
     def set_psf_band(self, lambdas_m=None, weights=None):

@@ -18,6 +18,8 @@
 // The scratch of a chunk is sized near the L2 capacity, but ncu --cache-control none shows that most of it is written
 // back to DRAM before the column pass reads it (profiles/r2_big_fft_l2.md): the passes are latency-bound, not DRAM-bound.
 #include <algorithm>
+#include <mutex>
+#include <string>
 
 #include "fft_big.cuh"
 
@@ -448,3 +450,85 @@ cudaError_t launch_psf(ao_geometry* g, const float* phase, bool api_layout, long
 }
 
 }  // namespace ao
+
+// ---- ao_psf_static: the science PSF of one direction with no allocation of any kind ----------------------------
+// For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it) and
+// therefore cannot lend a workspace either: the row pass's intermediate T[Np][M] lives in a file-scope device array
+// of AO_PSF_STATIC_MAX_BYTES (16 MiB, held by every GPU that loads the library until the process exits).  Same two
+// kernels as ao_psf (k_big_rows, k_big_cols<MODE 0>), one launch pair per step, one direction per call.
+// In host code `g_psf_static_scratch` is only a stand-in for the symbol: its device address is looked up once per
+// device with cudaGetSymbolAddress (that device current) and kept in g_psf_static_ptr[device].
+using namespace ao;
+
+static __device__ __align__(256) float2 g_psf_static_scratch[AO_PSF_STATIC_MAX_BYTES / sizeof(float2)];
+
+static constexpr int kMaxDevices = 64;
+static float2* g_psf_static_ptr[kMaxDevices];             // zero-initialised; written once per device
+static std::mutex g_psf_static_mutex;
+
+static cudaError_t psf_static_scratch(int device, float2** out)
+{
+    std::lock_guard<std::mutex> lock(g_psf_static_mutex);
+    if (!g_psf_static_ptr[device]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_psf_static_scratch);   // the calling thread's current device
+        if (e != cudaSuccess) return e;
+        g_psf_static_ptr[device] = static_cast<float2*>(p);
+    }
+    *out = g_psf_static_ptr[device];
+    return cudaSuccess;
+}
+
+extern "C" int ao_psf_static(ao_geometry* g, int direction, const float* phase_dev, int n_steps, float* psf_dev,
+                             int accumulate, void* cuda_stream)
+{
+    if (!g || !phase_dev || !psf_dev) { set_error("ao_psf_static: NULL argument"); return AO_ERR_INVALID_ARG; }
+    const int n_dir = (int)g->sci.src.size(), M = g->psf_fft;
+    if (n_dir == 0 || M == 0) { set_error("ao_psf_static: no science direction / psf_fft == 0"); return AO_ERR_INVALID_ARG; }
+    if (direction < 0 || direction >= n_dir || n_steps < 0) {
+        set_error("ao_psf_static: direction out of range or n_steps < 0"); return AO_ERR_INVALID_ARG;
+    }
+    const size_t need = sizeof(float2) * (size_t)g->Np * M;
+    if (need > (size_t)AO_PSF_STATIC_MAX_BYTES) {
+        set_error("ao_psf_static: pupil n * psf_fft * 8 = " + std::to_string(need) + " bytes exceeds the static scratch of " +
+                  std::to_string((size_t)AO_PSF_STATIC_MAX_BYTES) + " bytes (AO_PSF_STATIC_MAX_BYTES): use ao_psf with a workspace");
+        return AO_ERR_UNSUPPORTED;
+    }
+    if (g->device < 0 || g->device >= kMaxDevices) { set_error("ao_psf_static: device ordinal beyond 63"); return AO_ERR_UNSUPPORTED; }
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess && dev != g->device) e = cudaSetDevice(g->device);
+    if (e == cudaSuccess) e = cudaPeekAtLastError();
+    float2* scratch = nullptr;
+    if (e == cudaSuccess) e = psf_static_scratch(g->device, &scratch);
+    if (e != cudaSuccess) { set_error(std::string("ao_psf_static: ") + cudaGetErrorString(e)); return AO_ERR_CUDA; }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (n_steps == 0) {
+        if (!accumulate) e = cudaMemsetAsync(psf_dev, 0, sizeof(float) * (size_t)M * M, st);
+        if (e != cudaSuccess) { set_error(std::string("ao_psf_static: memset: ") + cudaGetErrorString(e)); return AO_ERR_CUDA; }
+        return AO_OK;
+    }
+    const int T = cols_threads_per_transform(M);
+    int C = 4;
+    while (T * C < 128) C *= 2;
+    while (T * C > 512) C /= 2;
+    for (int k = 0; k < n_steps && e == cudaSuccess; ++k) {
+        // the row pass writes every element of T[Np][M] the column pass reads: nothing has to start at zero
+        BigRowArgs r;
+        r.phase = phase_dev + (size_t)k * g->phase_elems_per_step; r.step_stride = g->phase_elems_per_step;
+        r.off = g->sci.d_off_api + direction; r.n_sel = 1;
+        r.amp = g->d_pupil_amp; r.valid = nullptr; r.n_sub = 1; r.n = g->Np;
+        r.tw = g->d_psf_tw; r.pre = g->d_psf_pre; r.T = scratch;
+        e = launch_rows(g->psf_log, r, g->Np, 1u, st);
+        if (e != cudaSuccess) break;
+        g->launches++;
+        BigColArgs c;
+        c.T = scratch; c.valid = nullptr; c.nsa = 1; c.n = g->Np; c.C = C; c.tw = g->d_psf_tw;
+        c.norm = g->sumA2 > 0 ? (float)(1.0 / ((double)M * M * g->sumA2)) : 0.0f;
+        c.beta = 1; c.P = 1; c.k0 = 0; c.n_dir = 1; c.ks = 1; c.accumulate = (accumulate || k > 0) ? 1 : 0; c.out = psf_dev;
+        e = launch_cols_psf(g->psf_log, c, (unsigned)(M / C), 1u, st);
+        if (e == cudaSuccess) g->launches++;
+    }
+    if (e != cudaSuccess) { set_error(std::string("ao_psf_static: launch: ") + cudaGetErrorString(e)); return AO_ERR_CUDA; }
+    return AO_OK;
+}
