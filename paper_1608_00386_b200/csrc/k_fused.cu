@@ -93,7 +93,10 @@ k_fused(const FusedArgs A)
     // ---- phase A: ray-trace of the 16 x 256 tile, two steps, into registers ----
     u64 acc[kKS * kTR];
     double refsum[2];                                      // unused: |FFT|^2 is piston-invariant per subaperture
-    trace2_tile<NT, false, ANYDU ? 1 : 0, true>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, refsum, it.cnt * n);
+    // a narrow work item (a run's tail) packs its columns on the first warps: pair distance 32 / 64 / 128 columns
+    const int ncols = it.cnt * n;
+    const int po = ncols > NT ? NT : (ncols > NT / 2 ? NT / 2 : NT / 4);
+    trace2_tile<NT, false, ANYDU ? 1 : 0, true>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, refsum, po);
     __syncthreads();                                       // stages are dead: shared memory becomes the exchange buffer
 
     // ---- phase B: image formation, one (subaperture row, column slot) round at a time ----
@@ -108,9 +111,9 @@ k_fused(const FusedArgs A)
         const int sp2 = hs / R2, h = hs - sp2 * R2;
         const int k = 2 * kp + sp2;
         const size_t set = (size_t)k * A.n_sel + si;
-        const int gs = c * K::GS + g;                      // subaperture within the item (column c*NT + tid)
+        const int gs = c * (po / n) + g;                   // subaperture within the item (column c * po + tid)
         const int q = it.q0 + gs, p = it.p + h;
-        const bool inb = gs < it.cnt && p < A.n_sub && k < A.n_steps;
+        const bool inb = tid < po && gs < it.cnt && p < A.n_sub && k < A.n_steps;
         const int sa = inb ? p * A.n_sub + q : 0;
         const bool active = inb && A.valid[sa] != 0;
         if (!__any_sync(0xffffffffu, active)) continue;

@@ -201,17 +201,19 @@ __device__ __forceinline__ void t2_march_unit(u64 (&acc)[kKS * kTR], const uint3
 // `dyn`: dynamic shared memory, 128-byte aligned: [ns][rows][pitch] floats, then trace2_sched_bytes(n_layers).
 // All NT threads call it.  On return every thread has finished reading the stages, but other warps may not
 // have: __syncthreads() before reusing the memory.
-// PARTIAL: only the first ncols_used columns of the tile are wanted (a work item with fewer subapertures than the
-// tile holds): a warp whose 32 columns tid and whose columns tid + NT all lie beyond them skips the row marches (its
-// acc stays zero); it still takes its producer turns and barrier arrivals.
+// PARTIAL: the tile is narrower than 2 NT columns (a work item with fewer subapertures than the tile holds): the thread's
+// second column is tid + pair_off instead of tid + NT (pair_off a multiple of 32, at most NT), so the first pair_off
+// threads cover columns 0 .. 2 pair_off - 1 and the warps from pair_off on skip the row marches (their acc stays zero);
+// they still take their producer turns and barrier arrivals.
 template <int NT, bool REFSUM, int MODE, bool PARTIAL = false>
 __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& sp, Trace2Shared& S, unsigned char* dyn,
                                             const int jfirst, const int ifirst, const long long step_first,
-                                            u64 (&acc)[kKS * kTR], double (&refsum)[2], const int ncols_used = 2 * NT)
+                                            u64 (&acc)[kKS * kTR], double (&refsum)[2], const int pair_off = NT)
 {
     constexpr int NCOL = 2 * NT;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const bool idle = PARTIAL && (int)(tid & ~31u) >= ncols_used;
+    const int PO = PARTIAL ? pair_off : NT;                  // column distance of the thread's packed pair
+    const bool idle = PARTIAL && tid >= PO;
     const int pitch = A.pitch, ns = A.ns;
     const int tile_floats = A.rows * pitch;
     float* tiles = reinterpret_cast<float*>(dyn);
@@ -384,25 +386,25 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             const UnitT u = *unit_of(T);
             const uint32_t b0 = tile_u + ((uint32_t)u.row[0] * kUnitPitch + (uint32_t)u.col[0]) * 4u;
             const uint32_t b1 = tile_u + ((uint32_t)u.row[1] * kUnitPitch + (uint32_t)u.col[1]) * 4u;
-            const float r0f = lds_f32(b0 + (uint32_t)(tid & ~31) * 4u), r1f = lds_f32(b0 + (uint32_t)((tid & ~31) + NT) * 4u);
+            const float r0f = lds_f32(b0 + (uint32_t)(tid & ~31) * 4u), r1f = lds_f32(b0 + (uint32_t)((tid & ~31) + PO) * 4u);
             const u64 ref = pack2(r0f, r1f);
             if (REFSUM) { refsum[0] += (double)r0f; refsum[1] += (double)r1f; }
             if (!AO_DBG_ON(A, 1) && !idle) {
-                t2_march_unit<0>(acc, b0 + (uint32_t)tid * 4u, b0 + (uint32_t)(tid + NT) * 4u, pack2(u.fx[0], u.fx[0]), ref, 1.0f - u.fy[0], u.fy[0]);
-                t2_march_unit<kTR>(acc, b1 + (uint32_t)tid * 4u, b1 + (uint32_t)(tid + NT) * 4u, pack2(u.fx[1], u.fx[1]), ref, 1.0f - u.fy[1], u.fy[1]);
+                t2_march_unit<0>(acc, b0 + (uint32_t)tid * 4u, b0 + (uint32_t)(tid + PO) * 4u, pack2(u.fx[0], u.fx[0]), ref, 1.0f - u.fy[0], u.fy[0]);
+                t2_march_unit<kTR>(acc, b1 + (uint32_t)tid * 4u, b1 + (uint32_t)(tid + PO) * 4u, pack2(u.fx[1], u.fx[1]), ref, 1.0f - u.fy[1], u.fy[1]);
             }
         } else {
         const uint32_t pb = (uint32_t)T.pitch * 4u;
         const u64 du64 = ((u64)(unsigned)T.du_hi << 32) | (u64)T.duf;
         const u64 uf0 = T.uf[0], uf1 = T.uf[1];
         const uint32_t tile_s = tiles_s + (uint32_t)stage * tile_bytes;
-        const u64 colA = (u64)(unsigned)tid * du64, colB = colA + (u64)NT * du64;
+        const u64 colA = (u64)(unsigned)tid * du64, colB = colA + (u64)(unsigned)PO * du64;
         const u64 colW = (u64)(unsigned)(tid & ~31) * du64;
         if (!AO_DBG_ON(A, 2)) mbar_wait(&S.full_bar[stage], par);
         const int ro0 = R0[stage * kKS], ro1 = R0[stage * kKS + 1];
         u64 ref;
         {
-            const u64 a0 = uf0 + colW, a1 = a0 + (u64)NT * du64;
+            const u64 a0 = uf0 + colW, a1 = a0 + (u64)(unsigned)PO * du64;
             const uint32_t rowb = tile_s + (uint32_t)ro0 * pb;
             const float r0f = lds_f32(rowb + (uint32_t)(a0 >> 32) * 4u), r1f = lds_f32(rowb + (uint32_t)(a1 >> 32) * 4u);
             ref = pack2(r0f, r1f);
