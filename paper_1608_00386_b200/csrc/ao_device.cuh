@@ -79,6 +79,46 @@ static __device__ __noinline__ int poisson_inv(const double mu, const double u)
 // decision is therefore the FP64 one of reading O5 in every case; the FP64 transcendental functions and the long FP64
 // recurrences, which were 5/6 of c2's step time, run for a few pixels per thousand.
 constexpr float kPoisMargin = 1.0e-4f;
+// mu < 12: a few terms from k = 0 (fp32 CDF within ~2e-6 of the FP64 one).  True if the decision *kout is certain.
+__device__ __forceinline__ bool poisson_small(const float muf, const float u, int* kout)
+{
+    int k = 0;
+    float p = expf(-muf), c = p, cprev = -1.0f;
+    while (u > c && k < 128) {
+        ++k;
+        p *= __fdividef(muf, (float)k);
+        cprev = c;
+        c += p;
+    }
+    *kout = k;
+    return k < 128 && u <= c - 0.2f * kPoisMargin && u > cprev + 0.2f * kPoisMargin;
+}
+// 12 <= mu < 1e6: from the mode, a walk of about one standard deviation.  True if the decision *kout is certain.
+__device__ __forceinline__ bool poisson_mode(const float muf, const float u, int* kout)
+{
+    const float m = floorf(muf), t = __fdividef(muf - m, m), inv_mu = __fdividef(1.0f, muf), im = __fdividef(1.0f, m);
+    // ln p_m = m ln(mu/m) - (mu - m) - ln sqrt(2 pi m) - 1/(12 m) + 1/(360 m^3): every term is small, fp32 keeps ~1e-6
+    const float im2 = im * im;
+    const float lnpm = m * (log1pf(t) - t) - 0.5f * logf(6.283185307f * m) - im * (0.0833333333f - im2 * (0.00277777778f - 0.000793650794f * im2));
+    const float pm = expf(lnpm);
+    // F(m) by the Peizer-Pratt normal approximation (absolute error at the mode, checked against scipy.stats.poisson.cdf:
+    // < 1e-5 for mu >= 8, 1.3e-6 for mu >= 16, < 2e-7 for mu in [32, 1e6]; it only has to stay far inside kPoisMargin):
+    //   z = (m + 2/3 - mu + 0.02/(m+1)) sqrt((1 + g(x)) / mu),  x = (m + 1/2)/mu,  g(x) = (1 - x^2 + 2x ln x)/(1 - x)^2,
+    // with g by its series in d = x - 1 (|d| <= 1/24): g = -d/3 + d^2/6 - d^3/10 + d^4/15.
+    const float d = (m + 0.5f - muf) * inv_mu;
+    const float g = d * (-0.333333333f + d * (0.166666667f + d * (-0.1f + d * 0.0666666667f)));
+    const float z = (m - muf + 0.666666667f + __fdividef(0.02f, m + 1.0f)) * sqrtf((1.0f + g) * inv_mu);
+    const float Fm = 0.5f * erfcf(-0.707106781f * z);
+    float p = pm;
+    float kf = m, c = Fm;
+    if (u <= c) {
+        while (kf > 0.0f && u <= c - p) { c -= p; p *= kf * inv_mu; kf -= 1.0f; }
+    } else {
+        while (u > c && kf < 2.0e6f) { kf += 1.0f; p *= __fdividef(muf, kf); c += p; if (p == 0.0f) break; }
+    }
+    *kout = (int)kf;
+    return u <= c - kPoisMargin && u > (c - p) + kPoisMargin;      // c = F(k), c - p = F(k - 1)
+}
 __device__ __forceinline__ int poisson_draw(const float I_times_photons, const uint32_t w)
 {
     const double ud = ((double)(w >> 8) + 0.5) * (1.0 / 16777216.0);      // exactly the oracle's u
@@ -87,39 +127,8 @@ __device__ __forceinline__ int poisson_draw(const float I_times_photons, const u
     if (!(muf > 0.0f)) return 0;
     int k = 0;
     bool sure = false;
-    if (muf < 12.0f) {                                     // a few terms from k = 0 (fp32 CDF within ~2e-6 of the FP64 one)
-        float p = expf(-muf), c = p, cprev = -1.0f;
-        while (u > c && k < 128) {
-            ++k;
-            p *= __fdividef(muf, (float)k);
-            cprev = c;
-            c += p;
-        }
-        sure = k < 128 && u <= c - 0.2f * kPoisMargin && u > cprev + 0.2f * kPoisMargin;
-    } else if (muf < 1.0e6f) {                             // from the mode: a walk of about one standard deviation
-        const float m = floorf(muf), t = __fdividef(muf - m, m), inv_mu = __fdividef(1.0f, muf), im = __fdividef(1.0f, m);
-        // ln p_m = m ln(mu/m) - (mu - m) - ln sqrt(2 pi m) - 1/(12 m) + 1/(360 m^3): every term is small, fp32 keeps ~1e-6
-        const float im2 = im * im;
-        const float lnpm = m * (log1pf(t) - t) - 0.5f * logf(6.283185307f * m) - im * (0.0833333333f - im2 * (0.00277777778f - 0.000793650794f * im2));
-        const float pm = expf(lnpm);
-        // F(m) by the Peizer-Pratt normal approximation (absolute error at the mode, checked against scipy.stats.poisson.cdf:
-        // < 1e-5 for mu >= 8, 1.3e-6 for mu >= 16, < 2e-7 for mu in [32, 1e6]; it only has to stay far inside kPoisMargin):
-        //   z = (m + 2/3 - mu + 0.02/(m+1)) sqrt((1 + g(x)) / mu),  x = (m + 1/2)/mu,  g(x) = (1 - x^2 + 2x ln x)/(1 - x)^2,
-        // with g by its series in d = x - 1 (|d| <= 1/24): g = -d/3 + d^2/6 - d^3/10 + d^4/15.
-        const float d = (m + 0.5f - muf) * inv_mu;
-        const float g = d * (-0.333333333f + d * (0.166666667f + d * (-0.1f + d * 0.0666666667f)));
-        const float z = (m - muf + 0.666666667f + __fdividef(0.02f, m + 1.0f)) * sqrtf((1.0f + g) * inv_mu);
-        const float Fm = 0.5f * erfcf(-0.707106781f * z);
-        float p = pm;
-        float kf = m, c = Fm;
-        if (u <= c) {
-            while (kf > 0.0f && u <= c - p) { c -= p; p *= kf * inv_mu; kf -= 1.0f; }
-        } else {
-            while (u > c && kf < 2.0e6f) { kf += 1.0f; p *= __fdividef(muf, kf); c += p; if (p == 0.0f) break; }
-        }
-        sure = u <= c - kPoisMargin && u > (c - p) + kPoisMargin;      // c = F(k), c - p = F(k - 1)
-        k = (int)kf;
-    }
+    if (muf < 12.0f) sure = poisson_small(muf, u, &k);
+    else if (muf < 1.0e6f) sure = poisson_mode(muf, u, &k);
     return sure ? k : poisson_inv(mu, ud);
 }
 
@@ -131,6 +140,55 @@ __device__ __forceinline__ float noisy_pixel(float I, const NoiseP& nz, uint32_t
     const int k = poisson_draw(nz.photons * I, w.x);
     const float z = sqrtf(-2.0f * logf(u24(w.y))) * cospif(2.0f * u24(w.z));
     return fmaf(nz.read_noise, z, (float)k);
+}
+
+// The same draws for NPX pixels per lane, with the long cases of the sampler shared out over the warp.  Every lane
+// draws its own dim pixels (mu < 12: a few fp32 terms); the bright ones (mode start, a walk of ~sqrt(mu) steps) and the
+// undecided ones (FP64 search) of all lanes are queued in `q` (shared memory of this warp, 32 NPX float2) and handed
+// out lane by lane, so the warp walks them with all lanes busy instead of once per pixel slot with the few lanes that
+// hold a bright pixel (c2: 3 to 7 of 32, and four unrolled copies of the sampler overflowed the instruction cache).
+// v[s] = noisy_pixel(v[s], ..., px[s], ...) for lanes with `on`; all 32 lanes must call it.
+template <int NPX>
+__device__ __forceinline__ void noisy_pixels_warp(float (&v)[NPX], const uint32_t (&px)[NPX], const bool on, const NoiseP& nz,
+                                                  const uint32_t sa, const uint32_t src, const uint32_t step, float2* q)
+{
+    const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
+    float z[NPX];
+    int k[NPX], slot[NPX];
+    int base = 0;
+#pragma unroll
+    for (int s = 0; s < NPX; ++s) {
+        const uint4 w = philox4x32_10(make_uint4(px[s], sa, src, step), nz.key0, nz.key1);
+        z[s] = sqrtf(-2.0f * logf(u24(w.y))) * cospif(2.0f * u24(w.z));
+        const float muf = nz.photons * v[s];
+        k[s] = 0;
+        bool pend = on && muf > 0.0f;
+        if (pend && muf < 12.0f) {
+            const float u = (float)(((double)(w.x >> 8) + 0.5) * (1.0 / 16777216.0));
+            pend = !poisson_small(muf, u, &k[s]);
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, pend);
+        slot[s] = pend ? base + __popc(m & lt) : -1;
+        if (pend) q[slot[s]] = make_float2(muf, __uint_as_float(w.x));
+        base += __popc(m);
+    }
+    __syncwarp();
+    for (int j = (int)lane; j < base; j += 32) {
+        const float2 e = q[j];
+        const float muf = e.x;
+        const double ud = ((double)(__float_as_uint(e.y) >> 8) + 0.5) * (1.0 / 16777216.0);
+        int kk = 0;
+        bool sure = false;
+        if (muf >= 12.0f && muf < 1.0e6f) sure = poisson_mode(muf, (float)ud, &kk);
+        if (!sure) kk = poisson_inv((double)muf, ud);
+        q[j].x = __int_as_float(kk);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int s = 0; s < NPX; ++s) {
+        if (slot[s] >= 0) k[s] = __float_as_int(q[slot[s]].x);
+        if (on) v[s] = fmaf(nz.read_noise, z[s], (float)k[s]);
+    }
 }
 
 // sin and cos of a phase of up to a few hundred radians: exact two-constant reduction to r = x/(2 pi) - k in

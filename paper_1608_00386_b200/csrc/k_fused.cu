@@ -225,6 +225,24 @@ k_fused(const FusedArgs A)
         constexpr int NPIX = P / BETA;                     // pixels kept per row after the exchange
         // detector rows of this thread: r = (b + hh n) / BETA ; columns cbase .. cbase + NPIX - 1
         float s = 0.0f, mx = 0.0f, my = 0.0f;
+        if (NOISE) {                                       // the thread's 2 NPIX pixels, long draws shared out over the warp
+            float nv[2 * NPIX];
+            uint32_t np[2 * NPIX];
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+                for (int i = 0; i < NPIX; ++i) {
+                    nv[hh * NPIX + i] = pixv[hh][i];
+                    np[hh * NPIX + i] = (uint32_t)(((b + hh * n) / BETA) * P + cbase + i);
+                }
+            __syncwarp();                                  // every lane has read its rows from xs: the warp's part is free
+            noisy_pixels_warp<2 * NPIX>(nv, np, active, A.nz, (uint32_t)sa, (uint32_t)src_index, (uint32_t)(A.T.step0 + k),
+                                        xch + (size_t)((tid & ~31) / n) * K::SUB_STRIDE);
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+                for (int i = 0; i < NPIX; ++i) pixv[hh][i] = nv[hh * NPIX + i];
+        }
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
             const int r = (b + hh * n) / BETA;
@@ -232,10 +250,6 @@ k_fused(const FusedArgs A)
             for (int i = 0; i < NPIX; ++i) {
                 float v = pixv[hh][i];
                 const int col = cbase + i;
-                if (NOISE) {
-                    if (active) v = noisy_pixel(v, A.nz, (uint32_t)(r * P + col), (uint32_t)sa, (uint32_t)src_index,
-                                                (uint32_t)(A.T.step0 + k));
-                }
                 if (A.images && active) A.images[(set * nsa + sa) * (P * P) + r * P + col] = v;
                 s += v;
                 mx = fmaf((float)col - 0.5f * (P - 1), v, mx);
