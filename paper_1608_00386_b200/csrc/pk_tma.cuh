@@ -106,6 +106,14 @@ __device__ __forceinline__ float lds_f32_imm(uint32_t addr)
     asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(addr), "n"(IMM));
     return v;
 }
+// Predicated tap pair: (s[addr], s[addr + 4]) if flag != 0, else zeros without touching shared memory (a predicated-off
+// load takes an issue slot but no shared-memory wavefront).
+__device__ __forceinline__ void lds_f32_pair_if(uint32_t addr, uint32_t flag, float& a, float& b)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %3, 0;\n\tmov.f32 %0, 0f00000000;\n\tmov.f32 %1, 0f00000000;\n\t"
+                 "@p ld.shared.f32 %0, [%2];\n\t@p ld.shared.f32 %1, [%2+4];\n\t}"
+                 : "=&f"(a), "=&f"(b) : "r"(addr), "r"(flag));
+}
 __device__ __forceinline__ float4 lds_f32x4(uint32_t addr)
 {
     float4 v;

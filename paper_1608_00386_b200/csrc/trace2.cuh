@@ -125,21 +125,31 @@ __device__ __forceinline__ void t2_march(u64 (&acc)[kKS * kTR], const uint32_t t
     }
 }
 
-// The same for ANY du > 0 (screen pixels per output sample): every output row builds both its top and its bottom
-// x-interpolated row from eight taps, acc_i += w0 X[r_i] + w1 X[r_i + 1]; about 1.5 times the work of t2_march,
-// still one basic block.  Used when a layer falls outside 1/2 <= du <= 1 (c4 at M = 16: the WFS grid is coarser
-// than the screens, du up to 1.5; low beacons).  Table entry: (w0, w1, byte offset of X[r_i] relative to X[r_0]).
+// The same for ANY du > 0 (screen pixels per output sample): acc_i += w0 X[r_i] + w1 X[r_i + 1].  Every output row builds
+// its bottom x-interpolated row from four taps; its top row is the previous row's bottom row when the march advanced by
+// exactly one screen row (for 1 <= du < 2 that is a fraction 2 - du of the rows), otherwise it is built from four more
+// taps, loaded under a warp-uniform predicate (predicated-off loads cost an issue slot, no shared-memory wavefront: at
+// du > 1 every tap load is two wavefronts, which is what bounds c4 at M = 16).  Still one basic block.  Used when a layer
+// falls outside 1/2 <= du <= 1 (c4 at M = 16: the WFS grid is coarser than the screens, du up to 1.5; low beacons).
+// Table entry: (w0, w1, byte offset of X[r_i] relative to X[r_0], flag: 1 = build the top row).
 template <int OFF>
 __device__ __forceinline__ void t2_march_any(u64 (&acc)[kKS * kTR], const uint32_t tp0, const uint32_t tp1, const uint32_t pb,
                                              const u64 fx, const u64 ref, const uint32_t wtab)
 {
+    u64 prev = 0ull;
 #pragma unroll
     for (int i = 0; i < kTR; ++i) {
         const float4 w = lds_f32x4(wtab + 16u * (uint32_t)i);
-        const uint32_t off = __float_as_uint(w.z);
-        const u64 top = t2_xrow(tp0 + off, tp1 + off, fx, ref);
+        const uint32_t off = __float_as_uint(w.z), flag = __float_as_uint(w.w);
         const u64 bot = t2_xrow(tp0 + off + pb, tp1 + off + pb, fx, ref);
+        float a0, a1, b0, b1;
+        lds_f32_pair_if(tp0 + off, flag, a0, a1);
+        lds_f32_pair_if(tp1 + off, flag, b0, b1);
+        const u64 p0 = pack2(a0, b0), p1 = pack2(a1, b1);
+        const u64 built = fma2(fx, sub2(p1, p0), sub2(p0, ref));
+        const u64 top = flag ? built : prev;
         acc[OFF + i] = fma2(pack2(w.y, w.y), bot, fma2(pack2(w.x, w.x), top, acc[OFF + i]));
+        prev = bot;
     }
 }
 
@@ -327,8 +337,10 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             } else if (MODE == 1) {
                 const long long ru = (long long)floor(v);                       // unclamped: rows may advance by 2 or more
                 const double fu = v - (double)ru;
+                const uint32_t build_top = (i == 0 || ru != rprev + 1) ? 1u : 0u;    // else the top row is the previous bottom row (rprev: unclamped)
                 Wt[stage * (kKS * kTR) + lane] = make_float4((float)(1.0 - fu), (float)fu,
-                                                              __uint_as_float((uint32_t)((int)(ru - r0) * pitch * 4)), 0.0f);
+                                                              __uint_as_float((uint32_t)((int)(ru - r0) * pitch * 4)),
+                                                              __uint_as_float(build_top));
             } else
             Wt[stage * (kKS * kTR) + lane] = make_float4((float)fy, adv ? w0 : 0.0f, adv ? 0.0f : w0,
                                                           __uint_as_float((uint32_t)((int)(r + 1 - r0) * pitch * 4)));
