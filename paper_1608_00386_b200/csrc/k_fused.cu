@@ -302,17 +302,22 @@ k_fused64(const FusedArgs A, const unsigned stash_off)
     float* stash = reinterpret_cast<float*>(smem + stash_off);     // [step][row < 16][column < 256]
 
     u64 acc[kKS * kTR];
-    double rs_top[2], rs_bot[2];
-    trace2_tile<NT, true, MODE>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, rs_top);
+    double rs_top[2] = {0.0, 0.0}, rs_bot[2] = {0.0, 0.0};
+#pragma unroll 1
+    for (int half = 0; half < 2; ++half) {                 // one copy of the march in the code: the kernel is 180 KB of SASS as it is
+        double rs[2];
+        trace2_tile<NT, true, MODE>(A.T, sp, S, smem, it.q0 * n, it.p * n + half * kTR, A.T.step0 + 2 * kp, acc, rs);
+        if (half == 0) {
+            rs_top[0] = rs[0]; rs_top[1] = rs[1];
 #pragma unroll
-    for (int i = 0; i < kKS * kTR; ++i) {
-        const float2 f = unpack2(acc[i]);
-        stash[i * kTileCols + tid] = f.x;
-        stash[i * kTileCols + NT + tid] = f.y;
+            for (int i = 0; i < kKS * kTR; ++i) {
+                const float2 f = unpack2(acc[i]);
+                stash[i * kTileCols + tid] = f.x;
+                stash[i * kTileCols + NT + tid] = f.y;
+            }
+        } else { rs_bot[0] = rs[0]; rs_bot[1] = rs[1]; }
+        __syncthreads();                                   // every warp has left the march: barriers and stages are re-armed / dead
     }
-    __syncthreads();                                       // every warp has left the first march: barriers and stages are re-armed
-    trace2_tile<NT, true, MODE>(A.T, sp, S, smem, it.q0 * n, it.p * n + kTR, A.T.step0 + 2 * kp, acc, rs_bot);
-    __syncthreads();                                       // stages are dead: shared memory becomes the exchange buffer
     const float dref[2] = {(float)(rs_top[0] - rs_bot[0]), (float)(rs_top[1] - rs_bot[1])};
 
     unsigned char* wbuf = smem + (size_t)warp * kF64Sub;
