@@ -70,15 +70,15 @@ struct __align__(16) LayerT {
     int tm;               // 1: the box does not wrap the screen edge and a tensor map exists: one TMA tensor copy
     int pitch, box_rows;  // shared-memory row pitch of this layer's box (the map's own box with a tensor copy) and its rows
     double du;            // screen pixels per output sample
-    double vrel[kKS];     // row coordinate of tile row 0 relative to box row 0
+    u64 vf[kKS];          // (row coordinate of tile row 0 - box row 0) 2^32
     u64 uf[kKS];          // (column coordinate of tile column 0 - box column 0) 2^32
 };
-// Unit march (du = 1): vrel / uf are replaced, in place, by what its consumers need: the box row of the top tap of tile
+// Unit march (du = 1): vf / uf are replaced, in place, by what its consumers need: the box row of the top tap of tile
 // row 0 and the box column of tile column 0 (per step), and the two fractional weights of the whole tile.
 struct UnitT { float fy[kKS], fx[kKS]; int row[kKS], col[kKS]; };
-static_assert(sizeof(UnitT) == sizeof(double) * kKS + sizeof(u64) * kKS, "UnitT overlays LayerT::vrel and LayerT::uf");
-__device__ __forceinline__ UnitT* unit_of(LayerT& T) { return reinterpret_cast<UnitT*>(&T.vrel[0]); }
-__device__ __forceinline__ const UnitT* unit_of(const LayerT& T) { return reinterpret_cast<const UnitT*>(&T.vrel[0]); }
+static_assert(sizeof(UnitT) == sizeof(u64) * kKS + sizeof(u64) * kKS, "UnitT overlays LayerT::vf and LayerT::uf");
+__device__ __forceinline__ UnitT* unit_of(LayerT& T) { return reinterpret_cast<UnitT*>(&T.vf[0]); }
+__device__ __forceinline__ const UnitT* unit_of(const LayerT& T) { return reinterpret_cast<const UnitT*>(&T.vf[0]); }
 
 struct __align__(16) Trace2Shared {
     uint64_t full_bar[kT2MaxStages], empty_bar[kT2MaxStages];
@@ -264,8 +264,9 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
             const long long c_lo = (long long)floor(uf[s]) & ~3LL;                         // 16-byte aligned start
             const long long c_hi = (long long)floor(fma((double)(NCOL - 1), du, uf[s])) + 2;
             const long long r_lo = (long long)floor(vf[s]);
-            long long r_hi = (long long)floor(fma((double)(kTR - 1), du, vf[s])) + 1;
-            if (MODE == 2) r_hi = max(r_hi, (long long)floor(fma((double)(kTR - 4), du, vf[s])) + 3);   // last group's fourth row
+            // 2^-20: the row table is built in 32.32 fixed point and may land one row further than the FP64 floor
+            long long r_hi = (long long)floor(fma((double)(kTR - 1), du, vf[s]) + 9.5367431640625e-7) + 1;
+            if (MODE == 2) r_hi = max(r_hi, (long long)floor(fma((double)(kTR - 4), du, vf[s]) + 9.5367431640625e-7) + 3);   // last group's fourth row
             if (s == 0 || c_lo < cmin) cmin = c_lo;
             if (s == 0 || c_hi > cmax) cmax = c_hi;
             if (s == 0 || r_lo < rmin) rmin = r_lo;
@@ -297,7 +298,7 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
 #pragma unroll
             for (int s = 0; s < kKS; ++s) {
                 T.uf[s] = __double2ull_rn((uf[s] - (double)cmin) * 4294967296.0);
-                T.vrel[s] = vf[s] - (double)rmin;
+                T.vf[s] = __double2ull_rn((vf[s] - (double)rmin) * 4294967296.0);
             }
         }
     }
@@ -310,41 +311,37 @@ __device__ __forceinline__ void trace2_tile(const Trace2Args& A, const SourceP& 
         const float* scr = T.scr;
         uint64_t* bar = &S.full_bar[stage];
         float* dst = tiles + (size_t)stage * tile_floats;
-        if (MODE != 3) {   // row table of this stage: lane = step * 16 + row (FP64); the unit march needs none
+        if (MODE != 3) {   // row table of this stage: lane = step * 16 + row; the unit march needs none
             static_assert(kKS * kTR == 32, "one lane per (step, row)");
+            // Row coordinates in 32.32 fixed point like the columns: row and fraction of tile row i are the two halves of
+            // vf + i du, exact to 2^-32 pixel per added du (the FP64 form of this table, floor and int <-> double conversions
+            // of 64-bit values, was 8 % of k_fused's stall samples: one warp per layer computes it inside the layer loop).
             const int s = lane / kTR, i = lane - s * kTR;
-            const double v = fma((double)i, T.du, T.vrel[s]);
-            long long r = (long long)floor(v);
-            const long long rprev = __shfl_up_sync(0xffffffffu, r, 1);
-            const long long r0 = __shfl_sync(0xffffffffu, r, s * kTR);
-            bool adv = true;
-            if (i > 0) {
-                if (r > rprev + 1) r = rprev + 1;                 // rounding across a cell edge: same value by continuity
-                adv = r != rprev;
-            }
-            const double fy = v - (double)r;
-            const float w0 = (float)(1.0 - fy);
+            const u64 du64t = ((u64)(unsigned)T.du_hi << 32) | (u64)T.duf;
+            const u64 V = T.vf[s] + (u64)(unsigned)i * du64t;
+            int r = (int)(V >> 32);
+            float fy = __uint2float_rn((unsigned)V) * 2.3283064365386963e-10f;            // may round to 1: same value by continuity
+            if (r + 1 >= T.rt) { r = T.rt - 2; fy = 1.0f; }                                // never a tap beyond the staged box
+            const int rprev = __shfl_up_sync(0xffffffffu, r, 1);
+            const int r0 = __shfl_sync(0xffffffffu, r, s * kTR);
+            const bool adv = i == 0 || r != rprev;
+            const float w0 = 1.0f - fy;
             if (MODE == 2) {
                 // rows in groups of four share four x-interpolated screen rows starting at the group's first top row
-                const long long ru = (long long)floor(v);
-                const long long rg = __shfl_sync(0xffffffffu, ru, lane & ~3);
-                const double fu = v - (double)ru;
-                const int j = (int)(ru - rg);                                    // 0 .. 2 for du <= 2/3
-                const float c0 = (float)(1.0 - fu), c1 = (float)fu;
+                const int rg = __shfl_sync(0xffffffffu, r, lane & ~3);
+                const int j = r - rg;                                            // 0 .. 2 for du <= 2/3
+                const float c0 = w0, c1 = fy;
                 Wt[stage * (kKS * kTR) + lane] = make_float4(j == 0 ? c0 : 0.0f, j == 0 ? c1 : (j == 1 ? c0 : 0.0f),
                                                               j == 1 ? c1 : (j == 2 ? c0 : 0.0f), j == 2 ? c1 : 0.0f);
-                if ((i & 3) == 0) G[(stage * kKS + s) * 4 + (i >> 2)] = (int)(ru - r0) * pitch * 4;
+                if ((i & 3) == 0) G[(stage * kKS + s) * 4 + (i >> 2)] = (r - r0) * pitch * 4;
             } else if (MODE == 1) {
-                const long long ru = (long long)floor(v);                       // unclamped: rows may advance by 2 or more
-                const double fu = v - (double)ru;
-                const uint32_t build_top = (i == 0 || ru != rprev + 1) ? 1u : 0u;    // else the top row is the previous bottom row (rprev: unclamped)
-                Wt[stage * (kKS * kTR) + lane] = make_float4((float)(1.0 - fu), (float)fu,
-                                                              __uint_as_float((uint32_t)((int)(ru - r0) * pitch * 4)),
+                const uint32_t build_top = (i == 0 || r != rprev + 1) ? 1u : 0u;   // else the top row is the previous bottom row
+                Wt[stage * (kKS * kTR) + lane] = make_float4(w0, fy, __uint_as_float((uint32_t)((r - r0) * pitch * 4)),
                                                               __uint_as_float(build_top));
             } else
-            Wt[stage * (kKS * kTR) + lane] = make_float4((float)fy, adv ? w0 : 0.0f, adv ? 0.0f : w0,
-                                                          __uint_as_float((uint32_t)((int)(r + 1 - r0) * pitch * 4)));
-            if (i == 0) R0[stage * kKS + s] = (int)r;
+            Wt[stage * (kKS * kTR) + lane] = make_float4(fy, adv ? w0 : 0.0f, adv ? 0.0f : w0,
+                                                          __uint_as_float((uint32_t)((r + 1 - r0) * pitch * 4)));
+            if (i == 0) R0[stage * kKS + s] = r;
         }
         __syncwarp();
         if (AO_DBG_ON(A, 2)) return;
