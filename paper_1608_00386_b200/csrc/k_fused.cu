@@ -94,9 +94,10 @@ k_fused(const FusedArgs A)
     u64 acc[kKS * kTR];
     double refsum[2];                                      // unused: |FFT|^2 is piston-invariant per subaperture
     // a narrow work item (a run's tail) packs its columns on the first warps: pair distance 32 / 64 / 128 columns
+    // (not in the ELONG instantiations: one more live value there costs 56 bytes of spills in the scatterer loop)
     const int ncols = it.cnt * n;
-    const int po = ncols > NT ? NT : (ncols > NT / 2 ? NT / 2 : NT / 4);
-    trace2_tile<NT, false, ANYDU ? 1 : 0, true>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, refsum, po);
+    const int po = ELONG ? NT : (ncols > NT ? NT : (ncols > NT / 2 ? NT / 2 : NT / 4));
+    trace2_tile<NT, false, ANYDU ? 1 : 0, !ELONG>(A.T, sp, S, smem, it.q0 * n, it.p * n, A.T.step0 + 2 * kp, acc, refsum, po);
     __syncthreads();                                       // stages are dead: shared memory becomes the exchange buffer
 
     // ---- phase B: image formation, one (subaperture row, column slot) round at a time ----
