@@ -11,7 +11,7 @@
 // CTA-wide barrier in the layer loop).  Each thread owns two columns (tid, tid + NT) packed in one 64-bit
 // register pair so that the inner loop is FFMA2 / FADD2.  Bilinear interpolation is separable: an output row
 // combines x-interpolated screen rows with warp-uniform y-weights.  Warp 0 writes, with each stage it issues,
-// the FP64 row table of that (layer, two steps): per output row the weights and the shared-memory offset of its
+// the row table of that (layer, two steps), built in 32.32 fixed point: per output row the weights and the shared-memory offset of its
 // bottom screen row, so the row march (t2_march) is branch-free straight-line code.
 // Column coordinates are 32.32 fixed point: cell and fraction of column j are the two halves of
 // uf + j * du (one IMAD.WIDE), exact to 2^-32 pixel at any screen coordinate.
