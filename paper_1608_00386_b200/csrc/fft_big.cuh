@@ -22,6 +22,15 @@ __device__ __forceinline__ float2 cmulf(const float2 a, const float2 b)
     return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
 }
 
+// Streaming load of the pass-1 intermediate: read once, strided by a whole row; kept out of L1 so that the twiddle table
+// (read by every butterfly of the later passes through L1) stays there.
+__device__ __forceinline__ float2 ldg_stream(const float2* p)
+{
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+
 // Stockham pass, load half: butterfly b = tb + q T (q < 16/R) reads points b + k M/R, k < R.
 template <int LOGM, int R, typename Load>
 __device__ __forceinline__ void pass_load(const int tb, float2 (&v)[16], Load&& ld)

@@ -112,7 +112,7 @@ k_big_cols(const BigColArgs A)
         for (int k = 0; k < A.ks; ++k) {
             const float2* Tb = A.T + ((size_t)(k * A.n_dir + b) * n) * M + m0 + c;
             big_fft<LOGM>(tb, sm, C, c, A.tw,
-                [&](int i) { return i < n ? __ldg(Tb + (size_t)i * M) : make_float2(0.0f, 0.0f); },
+                [&](int i) { return i < n ? ldg_stream(Tb + (size_t)i * M) : make_float2(0.0f, 0.0f); },
                 [&](int, const float2 x, int slot) { acc[slot] = fmaf(x.x, x.x, fmaf(x.y, x.y, acc[slot])); });
             __syncthreads();                                  // the next step overwrites the exchange buffer
         }
@@ -140,7 +140,7 @@ k_big_cols(const BigColArgs A)
         const float2* Tb = A.T + (size_t)b * n * M + m0 + c;
         float I[16];
         big_fft<LOGM>(tb, sm, C, c, A.tw,
-            [&](int i) { return i < n ? __ldg(Tb + (size_t)i * M) : make_float2(0.0f, 0.0f); },
+            [&](int i) { return i < n ? ldg_stream(Tb + (size_t)i * M) : make_float2(0.0f, 0.0f); },
             [&](int, const float2 x, int slot) { I[slot] = fmaf(x.x, x.x, x.y * x.y); });
         __syncthreads();                                      // every thread has finished reading the exchange buffer
         // intensities to shared memory as Ib[i][c] (replaying the index arithmetic of the last pass), then one

@@ -89,7 +89,7 @@ k_czt_cols(const CztArgs A)
     for (int k = 0; k < A.ks; ++k) {
         const float2* Tb = A.T + ((size_t)(k * A.n_dir + d) * A.Np) * A.M + m;
         big_fft<LOGL>(tb, sm, C, c, A.tw,
-            [&](int i) { return i < A.Np ? cmulf(__ldg(Tb + (size_t)i * A.M), __ldg(A.cin + i)) : make_float2(0.0f, 0.0f); },
+            [&](int i) { return i < A.Np ? cmulf(ldg_stream(Tb + (size_t)i * A.M), __ldg(A.cin + i)) : make_float2(0.0f, 0.0f); },
             [&](int i, const float2 x, int) { sm2[sidx(i)] = cconj(cmulf(x, __ldg(A.Hf + i))); });
         __syncthreads();
         const bool add = A.accumulate || k > 0;
