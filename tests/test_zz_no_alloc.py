@@ -79,3 +79,30 @@ def test_psf_static_refuses_sizes_beyond_its_static_array():
     assert err.value.status == 3                                     # AO_ERR_UNSUPPORTED
     assert "AO_PSF_STATIC_MAX_BYTES" in str(err.value) and str(cfg.pupil.n * cfg.psf_fft * 8) in str(err.value)
     assert np.all(dummy.cpu().numpy() == 0.0)
+
+
+def test_psf_static_replays_from_a_cuda_graph():
+    """The reason the entry point exists: a call captured into a CUDA graph (where cudaMalloc is forbidden) replays with
+    the same result as the workspace path, for two different phase buffers copied into the captured input."""
+    import torch
+    from paper_1608_00386_b200 import binding
+    cfg = inputs.make_config(4, n_sub=8, screen_n=512, n_steps=2, lgs_fft=16, n_layers=2)   # pupil 96, PSF FFT 256
+    M = cfg.psf_fft
+    geo = binding.Geometry(cfg, workspace_steps=2)
+    ph_a = geo.trace_layers(0, 2, cfg.dt_s)
+    ph_b = geo.trace_layers(40, 2, cfg.dt_s)
+    want_a = geo.psf(ph_a, 0, 2, cfg.dt_s)[0].clone()
+    want_b = geo.psf(ph_b, 40, 2, cfg.dt_s)[0].clone()
+    buf = ph_a.clone()
+    out = torch.zeros((M, M), dtype=torch.float32, device="cuda")
+    geo.psf_static(0, buf, 2, out)                                   # warm-up outside the capture (symbol address, attributes)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        geo.psf_static(0, buf, 2, out)
+    for ph, want in ((ph_b, want_b), (ph_a, want_a)):
+        buf.copy_(ph)
+        out.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        assert rel_l2(out.cpu().numpy(), want.cpu().numpy()) <= IMAGE_TOL
